@@ -1,0 +1,133 @@
+"""Process definitions and the helicity+colour summed, averaged |Mbar|^2 (oracle; test infrastructure).
+
+The five BASELINE.json configs plus the 2->2 processes used as pins.
+|Mbar|^2 follows Eq. 4 with the identical-particle factor of SURVEY 8c-A7.
+"""
+import itertools
+import math
+import numpy as np
+
+from . import feynman as fy
+
+
+class Process:
+    def __init__(self, name, initial, final, vertex_names):
+        self.name = name
+        self.initial, self.final = list(initial), list(final)
+        self.legs = [(x, 'in') for x in initial] + [(x, 'out') for x in final]
+        self.ext_fields = [x for x in initial] + [fy.anti(x) for x in final]
+        self.vertex_names = list(vertex_names)
+        self._cache = {}
+
+    @property
+    def n_ext(self):
+        return len(self.legs)
+
+    def helicities(self, leg):
+        name = self.legs[leg][0]
+        if fy.spin(name) == 'V' and fy._F[name][2] is not None:
+            return (-1, 0, 1)  # massive vector (never external in the configs)
+        return (-1, 1)
+
+    def ident_factor(self):
+        f = 1
+        for x in set(self.final):
+            f *= math.factorial(self.final.count(x))
+        return f
+
+    def avg_factor(self):
+        """1/(2*2) * 1/(n_a n_b) * 1/S_ident   (Eq. 4; A7)."""
+        na, nb = fy.coldim(self.initial[0]), fy.coldim(self.initial[1])
+        return 1.0 / (4.0 * na * nb * self.ident_factor())
+
+    def diagrams(self, par):
+        """Diagram list and the brute-force colour matrix between all (diagram, colour-structure) terms."""
+        key = tuple(sorted(par.items()))
+        if key not in self._cache:
+            verts = fy.build_vertices(par, self.vertex_names)
+            roots = fy.enumerate_diagrams(self.ext_fields, verts)
+            cols = []
+            for r in roots:
+                cols += [c.reshape(-1) for c in fy.root_colour(r)]
+            cmat = np.array(cols)  # [n_terms, prod(colour dims)]
+            cm = cmat @ np.conj(cmat.T)  # CM[l,l'] = sum_ext c_l conj(c_l')
+            self._cache[key] = (roots, cm, cmat)
+        return self._cache[key]
+
+
+def amplitudes(proc, p, par, hel, memo=None, kin=None):
+    """Kinematic amplitude of every (diagram, colour-structure) term for one helicity assignment: [n_terms, N]."""
+    roots, _, _ = proc.diagrams(par)
+    if kin is None:
+        kin = fy.Kinematics(proc, p, par)
+    out = []
+    for r in roots:
+        out += fy.root_amplitudes(r, hel, kin, memo)
+    return np.array(out)
+
+
+def me2(proc, p, par, per_helicity=False, batch=2048, wf_hook=None):
+    """|Mbar|^2 for momenta p [N, n_ext, 4] (GeV, physical E>0 for every leg).
+
+    wf_hook(kin), if given, may replace external wavefunctions in kin.wf before evaluation (used by the
+    Ward-identity pins: polarisation vector -> momentum)."""
+    p = np.asarray(p, dtype=float)
+    N = p.shape[0]
+    if N > batch:
+        parts = [me2(proc, p[i:i + batch], par, per_helicity, batch, wf_hook) for i in range(0, N, batch)]
+        return np.concatenate(parts, axis=-1)
+    roots, cm, _ = proc.diagrams(par)
+    kin = fy.Kinematics(proc, p, par)
+    if wf_hook is not None:
+        wf_hook(kin)
+    memo = {}
+    total = np.zeros(N)
+    per = {}
+    for hel in itertools.product(*[proc.helicities(i) for i in range(proc.n_ext)]):
+        a = amplitudes(proc, p, par, hel, memo, kin)  # [n_terms, N]
+        m2 = np.einsum('ln,lm,mn->n', a, cm, np.conj(a)).real
+        total += m2
+        if per_helicity:
+            per[hel] = m2 * proc.avg_factor()
+    if per_helicity:
+        return per
+    return total * proc.avg_factor()
+
+
+def me2_explicit_colour(proc, p, par):
+    """Same number by the literal double sum of Eq. 4: for every helicity AND every explicit external colour
+    assignment, add up the diagrams and square.  (Slower; used as a cross-check of the colour matrix.)"""
+    p = np.asarray(p, dtype=float)
+    roots, _, cmat = proc.diagrams(par)
+    kin = fy.Kinematics(proc, p, par)
+    total = np.zeros(p.shape[0])
+    for hel in itertools.product(*[proc.helicities(i) for i in range(proc.n_ext)]):
+        a = amplitudes(proc, p, par, hel, None, kin)  # [n_terms, N]
+        full = np.einsum('ln,lc->cn', a, cmat)  # amplitude for each explicit colour assignment c
+        total += np.sum(np.abs(full) ** 2, axis=0)
+    return total * proc.avg_factor()
+
+
+# ----------------------------------------------------------------------------- the five configs
+def config(i):
+    """BASELINE.json configs[i-1]; external leg order = initial then final as written there."""
+    if i == 1:
+        return Process('udx_epve', ['u', 'd~'], ['e+', 've'], ['udw', 'enw'])
+    if i == 2:
+        return Process('uux_epemg', ['u', 'u~'], ['e+', 'e-', 'g'], ['uug', 'uua', 'uuz', 'eea', 'eez'])
+    if i == 3:
+        return Process('udx_epvegg', ['u', 'd~'], ['e+', 've', 'g', 'g'],
+                       ['udw', 'enw', 'uug', 'ddg', 'ggg', 'gggg'])
+    if i == 4:
+        # decay-chain subset (A13): no gluon radiation off b, no non-resonant diagrams -> b has no g/a/z vertex
+        return Process('gg_ttxg_dilep', ['g', 'g'], ['b', 'e+', 've', 'b~', 'mu-', 'vm~', 'g'],
+                       ['ttg', 'ggg', 'gggg', 'tbw', 'enw', 'mnw'])
+    if i == 5:
+        return Process('udx_epveggg', ['u', 'd~'], ['e+', 've', 'g', 'g', 'g'],
+                       ['udw', 'enw', 'uug', 'ddg', 'ggg', 'gggg'])
+    raise ValueError(i)
+
+
+# sqrt(s_hat) [GeV] and number of events of each config (BASELINE.json)
+SQRT_S = {1: 80.0, 2: 500.0, 3: 1000.0, 4: 1500.0, 5: 2000.0}
+N_EVENTS = {1: 1 << 16, 2: 1 << 20, 3: 1 << 22, 4: 1 << 22, 5: 1 << 22}
