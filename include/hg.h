@@ -1,0 +1,166 @@
+/* hg.h -- C ABI of the B200 tree-level |M|^2 library (libhg.so).
+ *
+ * The hot path of arXiv:1305.0708 ("Fast computation of MadGraph amplitudes on GPU"): for a batch of
+ * phase-space points, evaluate the tree-level Standard Model matrix element squared, summed over
+ * helicities and colours and averaged over the initial state (Eq. 4-6), multiply by the
+ * phase-space weight and flux factor, and accumulate a Monte-Carlo cross section.
+ *
+ * Conventions common to every call
+ *   - units GeV, metric (+,-,-,-); momenta are physical (E > 0) for every external leg;
+ *   - "d_" pointers are DEVICE memory owned by the caller (the library never allocates per call and never
+ *     frees caller memory); "h_" pointers are HOST memory owned by the caller;
+ *   - momenta layout is structure-of-arrays p[leg][mu][event]: element (leg l, component mu, event e) sits
+ *     at index (l*4 + mu)*n + e; mu = 0..3 = (E, px, py, pz); leg order = initial then final state as
+ *     listed under hg_process below;
+ *   - precision HG_F64: every d_ array is double; HG_F32: every d_ array is float (accumulators stay
+ *     double);
+ *   - cuda_stream is a cudaStream_t passed as void* (NULL = default stream); calls are asynchronous on it
+ *     unless stated otherwise;
+ *   - every call returns 0 on success or a negative hg_status; the message of the last failure of a
+ *     context is available from hg_last_error().  Nothing throws across the ABI.  Arguments are validated
+ *     before any launch (NULL pointers, n < 0, unknown process/precision, parameters not set).  n == 0 is
+ *     a successful no-op.
+ *   - results depend only on (params, cuts, process, precision, seed, first_event, n, sqrt_s_hat): event
+ *     k always uses Philox counter k (reading SURVEY.md 8c-A15), so batches can be split or sharded.
+ */
+#ifndef HG_H
+#define HG_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct hg_ctx hg_ctx; /* opaque, library-owned */
+
+enum hg_status {
+  HG_OK = 0,
+  HG_EINVAL = -1,  /* bad argument */
+  HG_ENOPROC = -2, /* unknown process id */
+  HG_ECUDA = -3,   /* CUDA runtime error (text in hg_last_error) */
+  HG_ENOTSET = -4  /* hg_set_params has not been called on this context */
+};
+
+enum hg_precision { HG_F64 = 0, HG_F32 = 1 };
+
+/* The five BASELINE.json configs (workloads of PAPER.md:147-256, Eq. 12a, 13a, 17d).  Leg order:
+ *   HG_UDX_EPVE      u d~ -> e+ ve                                  (4 legs)
+ *   HG_UUX_EPEMG     u u~ -> e+ e- g                                (5 legs)
+ *   HG_UDX_EPVEGG    u d~ -> e+ ve g g                              (6 legs)
+ *   HG_GG_TTXG_DILEP g g  -> b e+ ve b~ mu- vm~ g   via t t~ g       (9 legs; decay-chain diagrams only)
+ *   HG_UDX_EPVEGGG   u d~ -> e+ ve g g g                            (7 legs)                         */
+enum hg_process {
+  HG_UDX_EPVE = 1,
+  HG_UUX_EPEMG = 2,
+  HG_UDX_EPVEGG = 3,
+  HG_GG_TTXG_DILEP = 4,
+  HG_UDX_EPVEGGG = 5
+};
+#define HG_N_PROCESS 5
+#define HG_MAX_EXT 9
+
+/* Standard Model inputs (paper's own: PAPER.md:1075; the configs override them).
+ * Derived inside hg_set_params with tree-level relations: sw2 = 1 - mw^2/mz^2, e = sqrt(4 pi/alpha_em_inv),
+ * gW = e/sw, gZ = e/(sw cw), gs = sqrt(4 pi alpha_s); FFV couplings follow Eq. 35.
+ * Widths enter only the propagator denominators (fixed width, reading SURVEY.md 8c-A4). */
+typedef struct {
+  double mz, mw, gz, gw; /* Z, W masses and widths */
+  double mt, gt;         /* top mass and width */
+  double mb;             /* bottom mass (0 in the configs) */
+  double mh, gh;         /* Higgs mass and width (library vertices only) */
+  double alpha_em_inv;   /* 1/alpha */
+  double alpha_s;        /* strong coupling, fixed */
+  int ckm_diagonal;      /* must be 1 (only the diagonal CKM is implemented) */
+} hg_params;
+
+/* Final-state cuts (Eq. 8-11; scope: SURVEY.md 8c-A11/A12).  A value <= 0 disables
+ * that cut.  A failing event keeps its place in the batch with weight 0 ("null value"). */
+typedef struct {
+  double pt_jet_min;  /* pT of every gluon jet > this */
+  double eta_jet_max; /* |eta| of every gluon jet < this */
+  double eta_lep_max; /* |eta| of every charged lepton < this */
+  double dr_jj_min;   /* Delta R (Eq. 9b) of every gluon pair > this */
+} hg_cuts;
+
+/* Static description of a generated process (from the process generator, step a0 of SURVEY.md 8a). */
+typedef struct {
+  int n_ext;          /* external legs */
+  int n_final;        /* final-state legs */
+  int n_hel_total;    /* 2^n_ext helicity combinations of Eq. 4 */
+  int n_hel_nonzero;  /* combinations that are not identically zero (the only ones evaluated) */
+  int n_diagrams;     /* topological Feynman diagrams */
+  int n_amplitudes;   /* diagrams after splitting four-gluon vertices into 3 colour structures (C.47-48) */
+  int n_flows;        /* colour-flow basis size = rank of the colour matrix */
+  int n_draws;        /* uniform random numbers per event used by the phase-space generator */
+  double avg_factor;  /* 1/(spin avg * colour avg * identical-particle factor), Eq. 4 + A7 */
+  double flops_f64;   /* algorithmic floating-point operations per event of hg_matrix_element (add, mul = 1,
+                         fma = 2, div, sqrt = 1), counted by running the generated code on a counting type */
+  double flops_ps;    /* same for phase-space generation + cuts (hg_gen_phase_space) */
+} hg_process_info_t;
+
+/* Create / destroy a context bound to one CUDA device.  hg_create selects the device for the calling
+ * thread (cudaSetDevice).  Returns HG_ECUDA if the device cannot be used. */
+int hg_create(hg_ctx** out, int cuda_device);
+void hg_destroy(hg_ctx* ctx);
+
+/* Text of the last error on this context (ctx-owned, valid until the next failing call).  ctx == NULL
+ * returns the text of the last hg_create failure. */
+const char* hg_last_error(const hg_ctx* ctx);
+
+/* Default inputs of BASELINE.json (MZ=91.1876, MW=80.419, GZ=2.441, GW=2.048, 1/alpha=132.507,
+ * mt=174.3, Gt=1.5, mb=0, alpha_s=0.118) and the default cuts of config `process`. */
+void hg_default_params(hg_params* out);
+int hg_default_cuts(int process, hg_cuts* out);
+
+/* Step a0 result.  Host only. */
+int hg_process_info(int process, hg_process_info_t* out);
+
+/* Set SM inputs and cuts; derives all couplings (host only, no launch).  cuts == NULL keeps each
+ * process' default cuts.  HG_EINVAL if a mass/width/alpha is not finite or positive where required,
+ * or ckm_diagonal != 1. */
+int hg_set_params(hg_ctx* ctx, const hg_params* par, const hg_cuts* cuts);
+
+/* Steps a1-a4: Philox4x32-10 uniforms -> flat RAMBO momenta at fixed sqrt_s_hat (config 4:
+ * Breit-Wigner mapped t, W masses, Eq. 27, massive RAMBO and nested two-body decays,
+ * Eq. 25-26) -> phase-space weight -> cuts.
+ *   d_p    [n_ext][4][n] out   momenta (SoA, see above), incoming legs = sqrt_s_hat/2 (1,0,0,+-1)
+ *   d_wps  [n] out             phase-space weight dPhi_n (includes the Breit-Wigner Jacobians ds/2pi)
+ *   d_pass [n] out or NULL     1 if the event passes the cuts else 0 (uint8)                         */
+int hg_gen_phase_space(hg_ctx* ctx, int process, int precision, uint64_t seed, uint64_t first_event,
+                       int64_t n, double sqrt_s_hat, void* d_p, void* d_wps, uint8_t* d_pass,
+                       void* cuda_stream);
+
+/* Steps a5-a8: |Mbar|^2 = avg_factor * sum_helicities sum_colours |sum_diagrams M|^2 (Eq. 4, 6) for every
+ * event of the batch (no cuts applied here).
+ *   d_p   [n_ext][4][n] in     momenta
+ *   d_me2 [n] out              |Mbar|^2 in GeV^(8 - 2 n_ext)                                         */
+int hg_matrix_element(hg_ctx* ctx, int process, int precision, int64_t n, const void* d_p, void* d_me2,
+                      void* cuda_stream);
+
+/* Same operation on HOST buffers: copies h_p to a context-owned device staging buffer (grown on demand,
+ * released by hg_destroy), runs hg_matrix_element and copies the result back; synchronises the stream. */
+int hg_matrix_element_host(hg_ctx* ctx, int process, int precision, int64_t n, const void* h_p,
+                           void* h_me2, void* cuda_stream);
+
+/* Steps a9-a10 on device arrays: w = pass * me2 * wps / (2 s_hat) * (hbar c)^2 [pb]; accumulates
+ * acc = (sum w, sum w^2, n, n_pass) in double.  d_pass may be NULL (all pass).  Synchronises the stream;
+ * acc is HOST memory, overwritten. */
+int hg_accumulate(hg_ctx* ctx, int precision, int64_t n, const void* d_me2, const void* d_wps,
+                  const uint8_t* d_pass, double sqrt_s_hat, double acc[4], void* cuda_stream);
+
+/* Steps a1-a10 fused in one kernel: each thread draws its event, builds momenta, applies the cuts,
+ * evaluates |Mbar|^2 only if it passes, forms w in pb and the block reduces (sum w, sum w^2, n_pass);
+ * nothing per-event touches HBM.  Synchronises the stream; acc (HOST, overwritten) = (sum w, sum w^2, n,
+ * n_pass).  sigma = acc[0]/acc[2]. */
+int hg_integrate_step(hg_ctx* ctx, int process, int precision, uint64_t seed, uint64_t first_event,
+                      int64_t n, double sqrt_s_hat, double acc[4], void* cuda_stream);
+
+/* Measured-peak helper for the roofline: runs a register-resident FMA chain on every SM
+ * and returns the achieved FLOP/s for the given precision in *flops_per_s.  Synchronises. */
+int hg_measure_fma_peak(hg_ctx* ctx, int precision, double* flops_per_s, void* cuda_stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HG_H */

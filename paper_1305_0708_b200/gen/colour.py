@@ -1,0 +1,188 @@
+"""Exact SU(3) colour algebra in the colour-flow (fundamental string) basis for the process generator.
+
+The paper keeps colour outside the HEGET functions: qqg amplitudes carry -T^a (Eq. 38), ggg
+carries i f^{abc} (Eq. 44), gggg three f f structures (Eq. 49 / C.48),
+and MG2CUDA multiplies the colour-basis amplitudes with a precomputed colour matrix.  Here
+every structure is rewritten on strings of generators along the (single) quark line,
+
+    i f^{abc} T^c = [T^a, T^b],
+
+so the colour of any subtree is a linear combination of WORDS (tuples of gluon leg numbers, in matrix-product
+order from the end of the fermion arrow to its start).  The colour matrix between two words is a trace, reduced
+exactly with the Fierz identity  T^a_ij T^a_kl = 1/2 (d_il d_jk - 1/N d_ij d_kl)  in rational arithmetic.
+
+Kinds of colour objects:
+  'none'  no colour content (leptons, electroweak bosons made of leptons)            words: ()
+  'col'   quark line open towards the parent at its END   (column spinor subtree)      words: tuple of legs
+  'row'   quark line open towards the parent at its START (row spinor subtree)
+  'adj'   gluon-type object X^a, represented by X = X^a T^a                           words: tuple of legs
+  'open'  gluon-type object X^a = (T^w1 .. T^a .. T^wn)_{ki} containing the whole quark line; the position of
+          the free adjoint index is the marker MARK inside the word
+  'line'  complete quark line (colour singlet towards the parent)
+"""
+from fractions import Fraction
+
+MARK = -1
+NC = 3
+
+
+class Col:
+    __slots__ = ('kind', 'terms')
+
+    def __init__(self, kind, terms):
+        self.kind = kind
+        self.terms = {w: c for w, c in terms.items() if c != 0}
+
+    def __repr__(self):
+        return 'Col(%s, %r)' % (self.kind, self.terms)
+
+    def scaled(self, s):
+        return Col(self.kind, {w: c * s for w, c in self.terms.items()})
+
+
+def _acc(d, w, c):
+    d[w] = d.get(w, 0) + c
+
+
+def leaf(kind, leg=None):
+    return Col(kind, {((leg,) if kind == 'adj' else ()): 1})
+
+
+def _subst(word, repl_words):
+    """Replace MARK in `word` by each (word, coeff) of repl_words."""
+    i = word.index(MARK)
+    return [(word[:i] + r + word[i + 1:], c) for r, c in repl_words]
+
+
+def f3(x, y):
+    """Colour of  i f^{xyz} X^x Y^y  as an object with free index z (used for ggg and, nested, for gggg)."""
+    out = {}
+    if x.kind == 'adj' and y.kind == 'adj':  # [X, Y]
+        for wx, cx in x.terms.items():
+            for wy, cy in y.terms.items():
+                _acc(out, wx + wy, cx * cy)
+                _acc(out, wy + wx, -cx * cy)
+        return Col('adj', out)
+    if x.kind == 'open' and y.kind == 'adj':  # i f^{xyz} T^x Y^y = [Y, T^z]
+        for wx, cx in x.terms.items():
+            for wy, cy in y.terms.items():
+                for w, c in _subst(wx, [(wy + (MARK,), 1), ((MARK,) + wy, -1)]):
+                    _acc(out, w, c * cx * cy)
+        return Col('open', out)
+    if x.kind == 'adj' and y.kind == 'open':  # i f^{xyz} X^x T^y = [T^z, X]
+        for wx, cx in x.terms.items():
+            for wy, cy in y.terms.items():
+                for w, c in _subst(wy, [((MARK,) + wx, 1), (wx + (MARK,), -1)]):
+                    _acc(out, w, c * cx * cy)
+        return Col('open', out)
+    raise ValueError('f3: unsupported colour kinds %s, %s' % (x.kind, y.kind))
+
+
+def contract(x, y):
+    """X^a Y^a for one 'open' and one 'adj' object -> complete line."""
+    if x.kind == 'adj' and y.kind == 'open':
+        x, y = y, x
+    if not (x.kind == 'open' and y.kind == 'adj'):
+        raise ValueError('contract: unsupported colour kinds %s, %s' % (x.kind, y.kind))
+    out = {}
+    for wx, cx in x.terms.items():
+        for w, c in _subst(wx, list(y.terms.items())):
+            _acc(out, w, c * cx)
+    return Col('line', out)
+
+
+def qqg(col, row, glu):
+    """Colour of the T^a_{ji} vertex given any two of (column quark, row quark, gluon) -> the third, or all
+    three -> complete line."""
+    out = {}
+    if col is not None and row is not None and glu is not None:
+        for wr, cr in row.terms.items():
+            for wg, cg in glu.terms.items():
+                for wc, cc in col.terms.items():
+                    _acc(out, wr + wg + wc, cr * cg * cc)
+        return Col('line', out)
+    if row is None:
+        for wg, cg in glu.terms.items():
+            for wc, cc in col.terms.items():
+                _acc(out, wg + wc, cg * cc)
+        return Col('col', out)
+    if col is None:
+        for wr, cr in row.terms.items():
+            for wg, cg in glu.terms.items():
+                _acc(out, wr + wg, cr * cg)
+        return Col('row', out)
+    for wr, cr in row.terms.items():
+        for wc, cc in col.terms.items():
+            _acc(out, wr + (MARK,) + wc, cr * cc)
+    return Col('open', out)
+
+
+def singlet(children):
+    """Colour of a colourless ('1' / delta) vertex: at most one quark line passes through."""
+    cols = [c for c in children if c.kind == 'col']
+    rows = [c for c in children if c.kind == 'row']
+    lines = [c for c in children if c.kind == 'line']
+    if any(c.kind in ('adj', 'open') for c in children):
+        raise ValueError('gluon-type object at a colourless vertex')
+    scale = 1
+    for c in children:
+        if c.kind == 'none':
+            scale *= c.terms[()]
+    if len(cols) + len(rows) + len(lines) == 0:
+        return Col('none', {(): scale})
+    if len(lines) == 1 and not cols and not rows:
+        return lines[0].scaled(scale)
+    if len(cols) == 1 and not rows and not lines:
+        return cols[0].scaled(scale)
+    if len(rows) == 1 and not cols and not lines:
+        return rows[0].scaled(scale)
+    if len(cols) == 1 and len(rows) == 1 and not lines:
+        out = {}
+        for wr, cr in rows[0].terms.items():
+            for wc, cc in cols[0].terms.items():
+                _acc(out, wr + wc, cr * cc * scale)
+        return Col('line', out)
+    raise ValueError('more than one quark line')
+
+
+# ----------------------------------------------------------------------------- traces
+def trace_pairs(word):
+    """Tr(T^{w1} ... T^{wm}) with every label appearing exactly twice (summed) -> Fraction."""
+    return _traces([tuple(word)])
+
+
+def _traces(cycles):
+    # product of traces; find a repeated label, apply Fierz
+    for ci, cyc in enumerate(cycles):
+        for i, a in enumerate(cyc):
+            # partner in the same cycle
+            for j in range(i + 1, len(cyc)):
+                if cyc[j] == a:
+                    x, y = cyc[i + 1:j], cyc[j + 1:] + cyc[:i]
+                    rest = cycles[:ci] + cycles[ci + 1:]
+                    # Tr(X T^a Y T^a) = 1/2 Tr X Tr Y - 1/(2N) Tr(XY)
+                    return (Fraction(1, 2) * _traces(rest + [x, y])
+                            - Fraction(1, 2 * NC) * _traces(rest + [x + y]))
+            # partner in another cycle
+            for cj in range(ci + 1, len(cycles)):
+                oth = cycles[cj]
+                if a in oth:
+                    j = oth.index(a)
+                    x = cyc[i + 1:] + cyc[:i]
+                    y = oth[j + 1:] + oth[:j]
+                    rest = [c for k, c in enumerate(cycles) if k not in (ci, cj)]
+                    # Tr(T^a X) Tr(T^a Y) = 1/2 Tr(XY) - 1/(2N) Tr X Tr Y
+                    return (Fraction(1, 2) * _traces(rest + [x + y])
+                            - Fraction(1, 2 * NC) * _traces(rest + [x, y]))
+    val = Fraction(1)
+    for cyc in cycles:
+        if len(cyc) != 0:
+            raise ValueError('unpaired label in trace')
+        val *= NC
+    return val
+
+
+def colour_matrix(words):
+    """C[w, w'] = sum over all colours of (T^w)_{ki} conj((T^w')_{ki}) = Tr(T^w (T^w')^dagger)."""
+    n = len(words)
+    return [[trace_pairs(tuple(words[a]) + tuple(reversed(words[b]))) for b in range(n)] for a in range(n)]

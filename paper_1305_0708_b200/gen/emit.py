@@ -1,0 +1,484 @@
+"""CUDA emitter: diagram list -> one fused per-process device function (steps a5-a8).
+
+Role of MG2CUDA's output stage (section 5.1, 5.4, 5.5), re-designed:
+  * helicity combinations that vanish identically are found at generation time by propagating chirality masks
+    through the diagrams (massless fermions keep one Weyl half; W couples to the left half only) and are never
+    evaluated;
+  * helicities of massless fermions are unrolled at generation time (they change the sparsity of the code),
+    helicities of gluons / massive particles are run-time loops, nested so that a sub-current is evaluated at the
+    loop depth of the deepest leg it depends on (values that depend on no looped leg are computed once);
+  * momenta of internal lines, their invariants and the propagator factors are helicity independent and are
+    computed once per event, before the helicity loops; invariants of massless pairs are formed from unit vectors
+    so that fp32 does not cancel for collinear pairs;
+  * amplitudes are added into colour-flow partial amplitudes jamp[f] with integer coefficients, and the colour
+    matrix (integers over a common denominator) is contracted per helicity combination.
+The paper's temporary-variable recycling is left to nvcc's register allocator: values are
+emitted in SSA form inside the loop scope where they live.
+"""
+import itertools
+from fractions import Fraction
+from math import factorial, gcd
+
+from . import colour as C
+from .diagrams import Diagrams, bits
+from .model import PARTICLES
+
+A, B, AB = 1, 2, 3
+GL, GR = 1, 2
+
+
+def _lcm(a, b):
+    return a * b // gcd(a, b)
+
+
+class Emitter:
+    def __init__(self, diag: Diagrams):
+        self.dg = diag
+        self.legs = diag.legs
+        self.static = [l.index for l in self.legs if l.particle.spin == 'F' and not l.particle.mass]
+        self.dynamic = [l.index for l in self.legs if l.index not in self.static]
+        self.nhel = {}
+        for l in self.legs:
+            p = l.particle
+            if p.spin == 'S':
+                self.nhel[l.index] = (0,)
+            elif p.spin == 'V' and p.mass:
+                self.nhel[l.index] = (-1, 0, 1)
+            else:
+                self.nhel[l.index] = (-1, 1)
+        self._analyse()
+
+    # ------------------------------------------------------------------ chirality masks
+    def _gmask(self, v):
+        return (GL if v.coup[0] else 0) | (GR if v.coup[1] else 0)
+
+    def _leaf_mask(self, nd, hel):
+        lg = self.legs[nd.leg]
+        p = lg.particle
+        if p.spin != 'F':
+            return AB
+        if p.mass:
+            return AB
+        nsf = self._nsf(lg)
+        colslot = A if hel[nd.leg] * nsf < 0 else B
+        if nd.wtype == 'col':
+            return colslot
+        return B if colslot == A else A
+
+    @staticmethod
+    def _nsf(lg):
+        return -1 if PARTICLES[lg.name].is_anti else +1
+
+    def _node_mask(self, nd, hel, memo):
+        """Non-zero slot mask of a node for the static helicity assignment hel (dict leg -> +-1); 0 = vanishes."""
+        key = (nd.uid, tuple(hel[l] for l in bits(nd.mask) if l in hel))
+        if key in memo:
+            return memo[key]
+        if nd.is_leaf:
+            r = self._leaf_mask(nd, hel)
+        else:
+            cm = [self._node_mask(ch, hel, memo) for ch in nd.children]
+            if 0 in cm:
+                r = 0
+            elif nd.vertex.kind in ('FFV', 'FFS'):
+                r = self._ff_mask(nd.vertex, dict(zip(nd.slots, cm)), nd.out_slot, bool(nd.particle.mass))
+            else:
+                r = AB
+        memo[key] = r
+        return r
+
+    def _ff_mask(self, v, by_slot, out_slot, massive):
+        g = self._gmask(v)
+        # FFV: gL pairs column slot A with row slot B; gR pairs column B with row A.
+        # FFS (Eq. 39): psibar (gL PL + gR PR) psi: gL pairs column A with row A; gR column B, row B.
+        scalar = v.kind == 'FFS'
+        if 0 in by_slot and 1 in by_slot:  # row and column given -> boson (or closed amplitude)
+            mo, mi = by_slot[0], by_slot[1]
+            rowL, rowR = (A, B) if scalar else (B, A)
+            ok = ((mi & A) and (mo & rowL) and (g & GL)) or ((mi & B) and (mo & rowR) and (g & GR))
+            return AB if ok else 0
+        if 1 in by_slot:  # column continues
+            mi = by_slot[1]
+            l, r = bool((mi & A) and (g & GL)), bool((mi & B) and (g & GR))
+            if not (l or r):
+                return 0
+            if massive:
+                return AB
+            if scalar:   # PL psi stays in A, then qslash moves it to B
+                return (B if l else 0) | (A if r else 0)
+            return (A if l else 0) | (B if r else 0)
+        mo = by_slot[0]  # row continues
+        if scalar:
+            l, r = bool((mo & A) and (g & GL)), bool((mo & B) and (g & GR))
+        else:
+            l, r = bool((mo & B) and (g & GL)), bool((mo & A) and (g & GR))
+        if not (l or r):
+            return 0
+        if massive:
+            return AB
+        if scalar:
+            return (B if l else 0) | (A if r else 0)
+        return (B if l else 0) | (A if r else 0)
+
+    def _root_nonzero(self, rt, hel, memo):
+        cm = [self._node_mask(ch, hel, memo) for ch in rt.children]
+        if 0 in cm:
+            return False
+        if rt.vertex.kind in ('FFV', 'FFS'):
+            return self._ff_mask(rt.vertex, dict(zip(rt.slots, cm)), -1, False) != 0
+        return True
+
+    def _analyse(self):
+        self.memo = {}
+        self.variants = []  # (hel dict for static legs, [non-zero roots])
+        for combo in itertools.product(*[self.nhel[l] for l in self.static]):
+            hel = dict(zip(self.static, combo))
+            roots = [r for r in self.dg.roots if self._root_nonzero(r, hel, self.memo)]
+            if roots:
+                self.variants.append((hel, roots))
+        ndyn = 1
+        for l in self.dynamic:
+            ndyn *= len(self.nhel[l])
+        self.n_hel_nonzero = len(self.variants) * ndyn
+        self.n_hel_total = 1
+        for l in self.legs:
+            self.n_hel_total *= len(self.nhel[l.index])
+
+    # ------------------------------------------------------------------ normalisation (Eq. 4; A7)
+    def avg_factor(self):
+        f = Fraction(1)
+        for l in self.legs:
+            if l.state == 'in':
+                f /= len(self.nhel[l.index])
+                f /= abs(l.particle.colour)
+        names = [l.name for l in self.legs if l.state == 'out']
+        for nm in set(names):
+            f /= factorial(names.count(nm))
+        return f
+
+    def colour_matrix(self):
+        flows = self.dg.flows()
+        cm = C.colour_matrix(flows)
+        den = 1
+        for row in cm:
+            for x in row:
+                den = _lcm(den, x.denominator)
+        return flows, [[int(x * den) for x in row] for row in cm], den
+
+
+# ====================================================================================== code generation
+def _popcount(m):
+    return bin(m).count('1')
+
+
+class CodeGen(Emitter):
+    """Emits `template <class T> HG_HD T me2_<name>(const Mom<T>* p, const Coup<T>& c)`."""
+
+    def generate(self):
+        self.need_K = set()       # masks whose summed momentum is needed
+        self.need_Kn = set()      # masks whose negated momentum is needed (row spinor propagators)
+        self.need_d = {}          # (mask, field) -> variable name of the propagator factor
+        self.need_rm2 = set()     # mass names whose 1/m^2 is needed
+        self.body = []
+        self.shared = {}          # key -> name of depth-0 values already emitted
+        self.shared_lines = []
+        dyn = self.dynamic
+        self.depth_of_leg = {l: i + 1 for i, l in enumerate(dyn)}
+        flows, cmat, cden = self.colour_matrix()
+        self.flows = flows
+        body = self.body
+        for vi, (hel, roots) in enumerate(self.variants):
+            self._emit_variant(vi, hel, roots, cmat)
+        out = []
+        out += self._preamble()
+        out += self.shared_lines
+        out.append('  T me = T(0);')
+        out += body
+        scale = self.avg_factor() / cden
+        out.append('  return me * T(%s);' % _lit(scale))
+        return out
+
+    # ------------------------------------------------------------------ helpers
+    def _depth(self, mask):
+        d = 0
+        for l in bits(mask):
+            d = max(d, self.depth_of_leg.get(l, 0))
+        return d
+
+    def _helcode(self, mask, hel):
+        return ''.join('p' if hel[l] > 0 else 'm' for l in bits(mask) if l in hel)
+
+    def _K(self, mask):
+        self.need_K.add(mask)
+        return 'K%d' % mask
+
+    def _Kn(self, mask):
+        self.need_K.add(mask)
+        self.need_Kn.add(mask)
+        return 'Kn%d' % mask
+
+    def _d(self, nd):
+        p = nd.particle
+        key = (nd.mask, p.mass, p.width, p.spin)
+        if key not in self.need_d:
+            self.need_d[key] = 'd%d_%s%s' % (nd.mask, p.spin.lower(), p.mass or '0')
+        return self.need_d[key]
+
+    def _mass(self, p):
+        return 'c.%s' % p.mass if p.mass else 'T(0)'
+
+    def _rm2(self, p):
+        if not p.mass:
+            return 'T(0)'
+        self.need_rm2.add(p.mass)
+        return 'rm2_%s' % p.mass
+
+    @staticmethod
+    def _cpl(name):
+        return 'c.%s' % name if name else 'T(0)'
+
+    def _name(self, nd, vi, hel):
+        if nd.is_leaf and nd.leg in self.depth_of_leg:
+            return 'x%d' % nd.leg
+        if self._depth(nd.mask) == 0:
+            return 's%d_%s' % (nd.uid, self._helcode(nd.mask, hel))
+        return 'v%d_%d' % (vi, nd.uid)
+
+    def _wtype_decl(self, nd):
+        return {'col': 'Sp<T>', 'row': 'Sp<T>', 'vec': 'Vc<T>', 'sca': 'cx<T>'}[nd.wtype]
+
+    # ------------------------------------------------------------------ one node
+    def _leaf_expr(self, nd, hel):
+        lg = self.legs[nd.leg]
+        p = lg.particle
+        if p.spin == 'F':
+            fn = 'ixxxx0' if nd.wtype == 'col' else 'oxxxx0'
+            return '%s<T>(p[%d], %d, %d)' % (fn, nd.leg, hel[nd.leg], self._nsf(lg))
+        raise NotImplementedError
+
+    def _node_expr(self, nd, vi, hel):
+        v = nd.vertex
+        by_slot = dict(zip(nd.slots, nd.children))
+        nm = lambda ch: self._name(ch, vi, hel)
+        mk = lambda ch: self._node_mask(ch, hel, self.memo)
+        p = nd.particle
+        massive = 'true' if p.mass else 'false'
+        if v.kind == 'FFV':
+            g = self._gmask(v)
+            gl, gr = self._cpl(v.coup[0]), self._cpl(v.coup[1])
+            if nd.out_slot == 0:    # remaining field is the row slot -> the column continues
+                col, vec = by_slot[1], by_slot[2]
+                return 'fvixxx<%d, %d, %s>(%s, %s, %s, %s, %s, %s, %s)' % (
+                    mk(col), g, massive, nm(col), nm(vec), gl, gr, self._K(nd.mask), self._mass(p), self._d(nd))
+            if nd.out_slot == 1:    # the row continues
+                row, vec = by_slot[0], by_slot[2]
+                return 'fvoxxx<%d, %d, %s>(%s, %s, %s, %s, %s, %s, %s)' % (
+                    mk(row), g, massive, nm(row), nm(vec), gl, gr, self._Kn(nd.mask), self._mass(p), self._d(nd))
+            row, col = by_slot[0], by_slot[1]
+            return 'jioxxx<%d, %d, %d, %s>(%s, %s, %s, %s, %s, %s, %s)' % (
+                mk(col), mk(row), g, massive, nm(col), nm(row), gl, gr, self._K(nd.mask), self._rm2(p), self._d(nd))
+        if v.kind == 'VVV':
+            a, b = by_slot[(nd.out_slot + 1) % 3], by_slot[(nd.out_slot + 2) % 3]
+            return 'jvvxxx<%s>(%s, %s, %s, %s, %s, %s, %s)' % (
+                massive, nm(a), nm(b), self._cpl(v.coup[0]), self._K(a.mask), self._K(b.mask), self._rm2(p),
+                self._d(nd))
+        if v.kind == 'VVVV':
+            if v.colour != 'ff':
+                raise NotImplementedError('electroweak four-boson vertex (K13, out of scope)')
+            kids = [by_slot[s] for s in sorted(by_slot)]
+            a, b, c3 = kids
+            x, y, z = {1: (a, b, c3), 2: (a, c3, b), 3: (b, c3, a)}[nd.struct]
+            return 'jgggxx(%s, %s, %s, %s, %s)' % (nm(x), nm(y), nm(z), self._cpl(v.coup[0]), self._d(nd))
+        raise NotImplementedError(v.kind)
+
+    def _root_expr(self, rt, vi, hel):
+        v = rt.vertex
+        by_slot = dict(zip(rt.slots, rt.children))
+        nm = lambda ch: self._name(ch, vi, hel)
+        mk = lambda ch: self._node_mask(ch, hel, self.memo)
+        if v.kind == 'FFV':
+            row, col, vec = by_slot[0], by_slot[1], by_slot[2]
+            return 'iovxxx<%d, %d, %d>(%s, %s, %s, %s, %s)' % (
+                mk(col), mk(row), self._gmask(v), nm(col), nm(row), nm(vec), self._cpl(v.coup[0]),
+                self._cpl(v.coup[1]))
+        if v.kind == 'VVV':
+            a, b, c3 = by_slot[0], by_slot[1], by_slot[2]
+            return 'vvvxxx(%s, %s, %s, %s, %s, %s, %s)' % (
+                nm(a), nm(b), nm(c3), self._cpl(v.coup[0]), self._K(a.mask), self._K(b.mask), self._K(c3.mask))
+        if v.kind == 'VVVV':
+            if v.colour != 'ff':
+                raise NotImplementedError('electroweak four-boson vertex (K13, out of scope)')
+            a, b, c3, d4 = [by_slot[s] for s in sorted(by_slot)]
+            x, y, z = {1: (a, b, c3), 2: (a, c3, b), 3: (b, c3, a)}[rt.struct]
+            return 'ggggxx(%s, %s, %s, %s, %s)' % (nm(x), nm(y), nm(z), nm(d4), self._cpl(v.coup[0]))
+        raise NotImplementedError(v.kind)
+
+    # ------------------------------------------------------------------ one static-helicity variant
+    def _emit_variant(self, vi, hel, roots, cmat):
+        dyn = self.dynamic
+        k = len(dyn)
+        levels = [[] for _ in range(k + 1)]   # lines per loop depth
+        done = set()
+
+        def need(nd):
+            """Emit nd (and, first, its children) in post-order."""
+            if nd.is_leaf and nd.leg in self.depth_of_leg:
+                return                      # dynamic leaf: declared by its loop header
+            dep = self._depth(nd.mask)
+            name = self._name(nd, vi, hel)
+            if dep == 0:
+                if name in self.shared:
+                    return
+            elif nd.uid in done:
+                return
+            for ch in nd.children:
+                need(ch)
+            expr = self._leaf_expr(nd, hel) if nd.is_leaf else self._node_expr(nd, vi, hel)
+            line = 'const %s %s = %s;' % (self._wtype_decl(nd), name, expr)
+            if dep == 0:
+                self.shared[name] = True
+                self.shared_lines.append('  ' + line)
+            else:
+                done.add(nd.uid)
+                levels[dep].append(line)
+
+        nf = len(self.flows)
+        fidx = {w: i for i, w in enumerate(self.flows)}
+        inner = levels[k]
+        # order the roots so that diagrams sharing deep sub-currents are adjacent
+        for rt in roots:
+            for ch in rt.children:
+                need(ch)
+            inner.append('{ const cx<T> a = %s;' % self._root_expr(rt, vi, hel))
+            for w, cf in sorted(rt.colour.terms.items()):
+                f = fidx[w]
+                if cf == 1:
+                    inner.append('  j%d = j%d + a;' % (f, f))
+                elif cf == -1:
+                    inner.append('  j%d = j%d - a;' % (f, f))
+                else:
+                    inner.append('  j%d = j%d + T(%d) * a;' % (f, f, cf))
+            inner.append('}')
+        # colour contraction (symmetric form)
+        tail = []
+        for f in range(nf):
+            terms = []
+            for g in range(f, nf):
+                cval = cmat[f][g] * (1 if g == f else 2)
+                if cval == 0:
+                    continue
+                terms.append('T(%d) * j%d' % (cval, g))
+            tail.append('{ const cx<T> t = %s; me += j%d.re * t.re + j%d.im * t.im; }' % (' + '.join(terms), f, f))
+        # assemble
+        b = self.body
+        ind = '  '
+        b.append(ind + '{  // static helicities: ' +
+                 ', '.join('%s(%d)=%+d' % (self.legs[l].name, l, h) for l, h in sorted(hel.items())))
+        ind += '  '
+        if k == 0:
+            b.append(ind + 'cx<T> ' + ', '.join('j%d = czero<T>()' % f for f in range(nf)) + ';')
+        for line in levels[0]:
+            b.append(ind + line)
+        for d in range(1, k + 1):
+            leg = dyn[d - 1]
+            lg = self.legs[leg]
+            nh = len(self.nhel[leg])
+            b.append(ind + '#pragma unroll 1')
+            b.append(ind + 'for (int h%d = 0; h%d < %d; ++h%d) {' % (leg, leg, nh, leg))
+            ind += '  '
+            b.append(ind + self._dyn_leaf_decl(lg))
+            if d == k:
+                b.append(ind + 'cx<T> ' + ', '.join('j%d = czero<T>()' % f for f in range(nf)) + ';')
+            for line in levels[d]:
+                b.append(ind + line)
+        for line in tail:
+            b.append(ind + line)
+        for d in range(k):
+            ind = ind[:-2]
+            b.append(ind + '}')
+        ind = ind[:-2]
+        b.append(ind + '}')
+
+    def _dyn_leaf_decl(self, lg):
+        p = lg.particle
+        i = lg.index
+        if p.spin == 'V' and not p.mass:
+            return 'const Vc<T> x%d = h%d ? vflip(e%d) : e%d;' % (i, i, i, i)
+        if p.spin == 'V':
+            nsv = -1 if lg.state == 'in' else 1
+            return 'const Vc<T> x%d = vxxxxx<T>(p[%d], c.%s, h%d - 1, %d);' % (i, i, p.mass, i, nsv)
+        if p.spin == 'F':
+            fn = 'oxxxxx' if p.is_anti else 'ixxxxx'
+            return 'const Sp<T> x%d = %s<T>(p[%d], c.%s, 2 * h%d - 1, %d);' % (i, fn, i, p.mass, i, self._nsf(lg))
+        return 'const cx<T> x%d = sxxxxx<T>();' % i
+
+    # ------------------------------------------------------------------ per-event, helicity independent part
+    def _preamble(self):
+        L = []
+        n = self.dg.n
+        sgn = {l.index: (1 if l.state == 'in' else -1) for l in self.legs}
+        # momenta of sub-sets (all-incoming: initial +p, final -p)
+        have = {}
+        for m in sorted(self.need_K, key=lambda m: (_popcount(m), m)):
+            self._emit_K(m, have, L, sgn)
+        for m in sorted(self.need_Kn):
+            L.append('  const Mom<T> Kn%d = -K%d;' % (m, m))
+        # invariants
+        pairs = set()
+        q2 = {}
+        for (m, mass, width, spin), name in sorted(self.need_d.items()):
+            if m not in q2:
+                use = m if _popcount(m) <= n - _popcount(m) else (self.dg.full & ~m)
+                q2[m] = use
+                ls = list(bits(use))
+                for a in range(len(ls)):
+                    for b2 in range(a + 1, len(ls)):
+                        pairs.add((ls[a], ls[b2]))
+        units = sorted({l for pr in pairs for l in pr if not self.legs[l].particle.mass})
+        for l in units:
+            L.append('  const Mom<T> n%d = unit0(p[%d]);' % (l, l))
+        for (a, b2) in sorted(pairs):
+            s = '' if sgn[a] * sgn[b2] > 0 else '-'
+            if not self.legs[a].particle.mass and not self.legs[b2].particle.mass:
+                L.append('  const T t%d_%d = %stwo_dot0(n%d, n%d);' % (a, b2, s, a, b2))
+            else:
+                L.append('  const T t%d_%d = %sT(2) * mdot(p[%d], p[%d]);' % (a, b2, s, a, b2))
+        for m, use in sorted(q2.items()):
+            ls = list(bits(use))
+            terms = ['t%d_%d' % (ls[a], ls[b2]) for a in range(len(ls)) for b2 in range(a + 1, len(ls))]
+            for l in ls:
+                if self.legs[l].particle.mass:
+                    terms.append('c.%s * c.%s' % (self.legs[l].particle.mass, self.legs[l].particle.mass))
+            L.append('  const T q2_%d = %s;' % (m, ' + '.join(terms)))
+        for mass in sorted(self.need_rm2):
+            L.append('  const T rm2_%s = hrcp(c.%s * c.%s);' % (mass, mass, mass))
+        for (m, mass, width, spin), name in sorted(self.need_d.items()):
+            sign = '' if spin == 'V' else '-'
+            den = 'q2_%d' % m if not mass else '(q2_%d - c.%s * c.%s)' % (m, mass, mass)
+            if width:
+                L.append('  const cx<T> %s = %scrcp(%s, c.%s * c.%s);' % (name, sign, den, mass, width))
+            else:
+                L.append('  const T %s = %shrcp(%s);' % (name, sign, den))
+        # polarisation vectors of looped massless vector legs (helicity +1; -1 by vflip)
+        for l in self.dynamic:
+            lg = self.legs[l]
+            if lg.particle.spin == 'V' and not lg.particle.mass:
+                L.append('  const Vc<T> e%d = vxxxxx<T>(p[%d], T(0), 1, %d);' % (l, l, -1 if lg.state == 'in' else 1))
+        return L
+
+    def _emit_K(self, m, have, L, sgn):
+        if m in have:
+            return
+        hi = max(bits(m))
+        rest = m & ~(1 << hi)
+        if rest == 0:
+            L.append('  const Mom<T> K%d = %sp[%d];' % (m, '' if sgn[hi] > 0 else '-', hi))
+        else:
+            self._emit_K(rest, have, L, sgn)
+            L.append('  const Mom<T> K%d = K%d %s p[%d];' % (m, rest, '+' if sgn[hi] > 0 else '-', hi))
+        have[m] = True
+
+
+def _lit(fr):
+    """Fraction -> C literal with full double precision."""
+    return repr(float(fr))
