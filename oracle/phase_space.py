@@ -47,6 +47,13 @@ def rambo_massless(u, n, rs):
         bq = np.sum(b * q[:, i, 1:], axis=1)
         p[:, i, 0] = x * (g * q[:, i, 0] + bq)
         p[:, i, 1:] = x[:, None] * (q[:, i, 1:] + b * q[:, i, 0][:, None] + (a * bq)[:, None] * b)
+    # Reading A16b.  The conformal map above is ill-conditioned (~ (Q0/M)^2 roundings) when the q_i are
+    # nearly collinear, so its output satisfies sum p = (rs, 0) and p_i^2 = 0 only to that accuracy.  The point is
+    # put back on the constraint surface exactly: the last 3-momentum closes the sum, every energy is |p_i|, and
+    # one common factor restores sum E = rs.  This moves the point by no more than the rounding it already had.
+    p[:, n - 1, 1:] = -p[:, :n - 1, 1:].sum(axis=1)
+    p[:, :, 0] = np.sqrt(np.sum(p[:, :, 1:] ** 2, axis=2))
+    p *= (rs / p[:, :, 0].sum(axis=1))[:, None, None]
     vol = (math.pi / 2.0) ** (n - 1) * rs ** (2 * n - 4) / (math.factorial(n - 1) * math.factorial(n - 2)) \
         * TWO_PI ** (4 - 3 * n)
     return p, np.full(N, vol)
@@ -83,13 +90,15 @@ def bw_mass(u, m, gam):
     return s, jac
 
 
-def boost(pr, P, M):
-    """Boost pr (given in the rest frame of a particle of mass M) to the frame where that particle has momentum P."""
+def boost(pr, P, M, msq):
+    """Boost pr (given in the rest frame of a particle of mass M) to the frame where that particle has momentum P.
+    The boosted energy (P.pr)/M fixes the 3-momentum; the returned energy is then taken from the mass-shell
+    condition E = sqrt(|p|^2 + msq) (reading A16b), equal to it up to rounding."""
     e = (P[:, 0] * pr[:, 0] + np.sum(P[:, 1:] * pr[:, 1:], axis=1)) / M
     fac = (e + pr[:, 0]) / (P[:, 0] + M)
     out = np.empty_like(pr)
-    out[:, 0] = e
     out[:, 1:] = pr[:, 1:] + fac[:, None] * P[:, 1:]
+    out[:, 0] = np.sqrt(np.sum(out[:, 1:] ** 2, axis=1) + msq)
     return out
 
 
@@ -104,7 +113,7 @@ def two_body(P, M2, m1sq, m2sq, uc, uf):
     d = np.stack([st * np.cos(f), st * np.sin(f), c], axis=1) * pst[:, None]
     p1 = np.concatenate([np.sqrt(pst ** 2 + m1sq)[:, None], d], axis=1)
     p2 = np.concatenate([np.sqrt(pst ** 2 + m2sq)[:, None], -d], axis=1)
-    return boost(p1, P, M), boost(p2, P, M), pst / (4.0 * math.pi * M)
+    return boost(p1, P, M, m1sq), boost(p2, P, M, m2sq), pst / (4.0 * math.pi * M)
 
 
 N_FINAL = {1: 2, 2: 3, 3: 4, 5: 5}

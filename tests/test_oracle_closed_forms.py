@@ -192,8 +192,8 @@ def test_cfg3_soft_gluon_limit_pins_normalisation():
         M = np.sqrt(d(tot, tot))
         Pm = tot.copy()
         Pm[:, 1:] *= -1.0  # boosting with -P brings P to rest
-        pf = np.stack([ps.boost(pf[:, i], Pm, M) for i in range(3)], 1)
-        k = ps.boost(k, Pm, M)
+        pf = np.stack([ps.boost(pf[:, i], Pm, M, 0.0) for i in range(3)], 1)
+        k = ps.boost(k, Pm, M, 0.0)
         pa = np.stack([M / 2, 0 * M, 0 * M, M / 2], 1)
         pb = np.stack([M / 2, 0 * M, 0 * M, -M / 2], 1)
         p4 = np.stack([pa, pb, pf[:, 0], pf[:, 1], pf[:, 2], k], 1)
