@@ -1,0 +1,227 @@
+"""Thin ctypes binding of libhg.so (include/hg.h): argument marshalling only, same names as the C ABI.
+
+PyTorch supplies device memory and streams (`tensor.data_ptr()`, `torch.cuda.current_stream().cuda_stream`); every
+step of the path runs in the library's kernels.  There is no CPU fallback: importing works without a GPU (the
+library loads and its host-only calls work), any compute call without a CUDA device fails loudly.
+"""
+import ctypes as C
+import os
+
+import torch
+
+HG_F64, HG_F32 = 0, 1
+HG_UDX_EPVE, HG_UUX_EPEMG, HG_UDX_EPVEGG, HG_GG_TTXG_DILEP, HG_UDX_EPVEGGG = 1, 2, 3, 4, 5
+PROCESSES = (1, 2, 3, 4, 5)
+HG_OK, HG_EINVAL, HG_ENOPROC, HG_ECUDA, HG_ENOTSET = 0, -1, -2, -3, -4
+
+# symbols include/hg.h declares (checked by tests/test_abi.py)
+SYMBOLS = ('hg_create', 'hg_destroy', 'hg_last_error', 'hg_default_params', 'hg_default_cuts', 'hg_process_info',
+           'hg_set_params', 'hg_gen_phase_space', 'hg_matrix_element', 'hg_matrix_element_host', 'hg_accumulate',
+           'hg_integrate_step', 'hg_measure_fma_peak')
+
+
+class hg_params(C.Structure):
+    _fields_ = [(n, C.c_double) for n in ('mz', 'mw', 'gz', 'gw', 'mt', 'gt', 'mb', 'mh', 'gh', 'alpha_em_inv',
+                                          'alpha_s')] + [('ckm_diagonal', C.c_int)]
+
+
+class hg_cuts(C.Structure):
+    _fields_ = [(n, C.c_double) for n in ('pt_jet_min', 'eta_jet_max', 'eta_lep_max', 'dr_jj_min')]
+
+
+class hg_process_info_t(C.Structure):
+    _fields_ = [(n, C.c_int) for n in ('n_ext', 'n_final', 'n_hel_total', 'n_hel_nonzero', 'n_diagrams',
+                                       'n_amplitudes', 'n_flows', 'n_draws')] + \
+               [(n, C.c_double) for n in ('avg_factor', 'flops_f64', 'flops_ps')]
+
+
+class HgError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__('hg error %d: %s' % (code, msg))
+        self.code = code
+
+
+_LIB = None
+
+
+def lib_path():
+    return os.path.join(os.path.dirname(os.path.abspath(__file__)), 'libhg.so')
+
+
+def load():
+    """Load libhg.so (built in-tree by paper_1305_0708_b200.build).  Raises if it is missing: no fallback."""
+    global _LIB
+    if _LIB is not None:
+        return _LIB
+    path = lib_path()
+    if not os.path.exists(path):
+        raise ImportError('%s not found: run `python -m paper_1305_0708_b200.build` (nvcc, sm_100a)' % path)
+    L = C.CDLL(path)
+    vp, i32, i64, u64, dbl = C.c_void_p, C.c_int, C.c_int64, C.c_uint64, C.c_double
+    L.hg_create.argtypes = [C.POINTER(vp), i32]
+    L.hg_destroy.argtypes = [vp]
+    L.hg_destroy.restype = None
+    L.hg_last_error.argtypes = [vp]
+    L.hg_last_error.restype = C.c_char_p
+    L.hg_default_params.argtypes = [C.POINTER(hg_params)]
+    L.hg_default_params.restype = None
+    L.hg_default_cuts.argtypes = [i32, C.POINTER(hg_cuts)]
+    L.hg_process_info.argtypes = [i32, C.POINTER(hg_process_info_t)]
+    L.hg_set_params.argtypes = [vp, C.POINTER(hg_params), C.POINTER(hg_cuts)]
+    L.hg_gen_phase_space.argtypes = [vp, i32, i32, u64, u64, i64, dbl, vp, vp, vp, vp]
+    L.hg_matrix_element.argtypes = [vp, i32, i32, i64, vp, vp, vp]
+    L.hg_matrix_element_host.argtypes = [vp, i32, i32, i64, vp, vp, vp]
+    L.hg_accumulate.argtypes = [vp, i32, i64, vp, vp, vp, dbl, C.POINTER(dbl), vp]
+    L.hg_integrate_step.argtypes = [vp, i32, i32, u64, u64, i64, dbl, C.POINTER(dbl), vp]
+    L.hg_measure_fma_peak.argtypes = [vp, i32, C.POINTER(dbl), vp]
+    _LIB = L
+    return L
+
+
+def hg_default_params():
+    p = hg_params()
+    load().hg_default_params(C.byref(p))
+    return p
+
+
+def hg_default_cuts(process):
+    c = hg_cuts()
+    rc = load().hg_default_cuts(process, C.byref(c))
+    if rc != HG_OK:
+        raise HgError(rc, 'unknown process id')
+    return c
+
+
+def hg_process_info(process):
+    info = hg_process_info_t()
+    rc = load().hg_process_info(process, C.byref(info))
+    if rc != HG_OK:
+        raise HgError(rc, 'unknown process id')
+    return {n: getattr(info, n) for n, _ in hg_process_info_t._fields_}
+
+
+def _dtype(precision):
+    return torch.float64 if precision == HG_F64 else torch.float32
+
+
+def _stream(stream):
+    if stream is None:
+        return torch.cuda.current_stream().cuda_stream
+    return stream.cuda_stream if hasattr(stream, 'cuda_stream') else int(stream)
+
+
+def _ptr(t):
+    return None if t is None else C.c_void_p(t.data_ptr())
+
+
+class Context:
+    """hg_ctx with the C calls as methods of the same names."""
+
+    def __init__(self, device=0, params=None, cuts=None):
+        self._L = load()
+        if not torch.cuda.is_available():
+            raise RuntimeError('paper_1305_0708_b200 needs a CUDA device: there is no CPU path')
+        h = C.c_void_p()
+        rc = self._L.hg_create(C.byref(h), int(device))
+        if rc != HG_OK:
+            raise HgError(rc, self._L.hg_last_error(None).decode())
+        self._h = h
+        self.device = torch.device('cuda', int(device))
+        self.hg_set_params(params if params is not None else hg_default_params(), cuts)
+
+    def close(self):
+        if getattr(self, '_h', None):
+            self._L.hg_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _check(self, rc):
+        if rc != HG_OK:
+            raise HgError(rc, self._L.hg_last_error(self._h).decode())
+
+    def hg_set_params(self, params, cuts=None):
+        self._check(self._L.hg_set_params(self._h, C.byref(params), C.byref(cuts) if cuts is not None else None))
+
+    def _check_tensor(self, t, precision, numel, name, dtype=None):
+        dtype = dtype or _dtype(precision)
+        if t.device.type != 'cuda' or t.dtype != dtype or not t.is_contiguous() or t.numel() != numel:
+            raise ValueError('%s must be a contiguous CUDA %s tensor with %d elements' % (name, dtype, numel))
+
+    def hg_gen_phase_space(self, process, precision, seed, first_event, n, sqrt_s_hat, p=None, wps=None,
+                           passed=None, stream=None, want_pass=True):
+        """Returns (p [n_ext,4,n], wps [n], pass [n] uint8).  Buffers are allocated with torch if not given."""
+        n_ext = hg_process_info(process)['n_ext']
+        dt = _dtype(precision)
+        if p is None:
+            p = torch.empty((n_ext, 4, n), dtype=dt, device=self.device)
+        if wps is None:
+            wps = torch.empty((n,), dtype=dt, device=self.device)
+        if passed is None and want_pass:
+            passed = torch.empty((n,), dtype=torch.uint8, device=self.device)
+        self._check_tensor(p, precision, n_ext * 4 * n, 'p')
+        self._check_tensor(wps, precision, n, 'wps')
+        if passed is not None:
+            self._check_tensor(passed, precision, n, 'pass', torch.uint8)
+        self._check(self._L.hg_gen_phase_space(self._h, process, precision, seed, first_event, n, sqrt_s_hat,
+                                               _ptr(p), _ptr(wps), _ptr(passed), _stream(stream)))
+        return p, wps, passed
+
+    def hg_matrix_element(self, process, precision, p, me2=None, stream=None):
+        """p: CUDA tensor [n_ext, 4, n] (SoA).  Returns me2 [n]."""
+        n_ext = hg_process_info(process)['n_ext']
+        n = p.numel() // (4 * n_ext)
+        self._check_tensor(p, precision, n_ext * 4 * n, 'p')
+        if me2 is None:
+            me2 = torch.empty((n,), dtype=_dtype(precision), device=p.device)
+        self._check_tensor(me2, precision, n, 'me2')
+        self._check(self._L.hg_matrix_element(self._h, process, precision, n, _ptr(p), _ptr(me2), _stream(stream)))
+        return me2
+
+    def hg_matrix_element_host(self, process, precision, p, me2=None, stream=None):
+        """p: HOST tensor [n_ext, 4, n] (pinned for full speed).  Returns a host tensor me2 [n]; synchronises."""
+        n_ext = hg_process_info(process)['n_ext']
+        n = p.numel() // (4 * n_ext)
+        dt = _dtype(precision)
+        if p.device.type != 'cpu' or p.dtype != dt or not p.is_contiguous():
+            raise ValueError('p must be a contiguous host %s tensor' % dt)
+        if me2 is None:
+            me2 = torch.empty((n,), dtype=dt).pin_memory()
+        self._check(self._L.hg_matrix_element_host(self._h, process, precision, n, _ptr(p), _ptr(me2),
+                                                   _stream(stream)))
+        return me2
+
+    def hg_accumulate(self, precision, me2, wps, passed, sqrt_s_hat, stream=None):
+        n = me2.numel()
+        self._check_tensor(me2, precision, n, 'me2')
+        self._check_tensor(wps, precision, n, 'wps')
+        if passed is not None:
+            self._check_tensor(passed, precision, n, 'pass', torch.uint8)
+        acc = (C.c_double * 4)()
+        self._check(self._L.hg_accumulate(self._h, precision, n, _ptr(me2), _ptr(wps), _ptr(passed), sqrt_s_hat,
+                                          acc, _stream(stream)))
+        return tuple(acc)
+
+    def hg_integrate_step(self, process, precision, seed, first_event, n, sqrt_s_hat, stream=None):
+        """Returns (sum w, sum w^2, n, n_pass), w in pb."""
+        acc = (C.c_double * 4)()
+        self._check(self._L.hg_integrate_step(self._h, process, precision, seed, first_event, n, sqrt_s_hat, acc,
+                                              _stream(stream)))
+        return tuple(acc)
+
+    def hg_measure_fma_peak(self, precision, stream=None):
+        out = C.c_double()
+        self._check(self._L.hg_measure_fma_peak(self._h, precision, C.byref(out), _stream(stream)))
+        return out.value
+
+
+def sigma(acc):
+    """sigma = sum w / N and its Monte-Carlo standard error from (sum w, sum w^2, N, N_pass)."""
+    sw, sw2, n, _ = acc
+    s = sw / n
+    var = max(sw2 / n - s * s, 0.0) / max(n - 1.0, 1.0)
+    return s, var ** 0.5

@@ -1,0 +1,444 @@
+// hg_api.cu -- the C-ABI boundary of libhg.so (include/hg.h): argument checking, per-call constants, dispatch to
+// the per-process translation units, the process-independent kernels (accumulate, finalize, FMA peak).
+#include <math.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <string>
+
+#include "hg_couplings.h"
+#include "hg_host_setup.h"
+#include "hg_internal.h"
+
+namespace hg {
+
+static const ProcVTable* vtable(int process) {
+  switch (process) {
+    case HG_UDX_EPVE: return &hg_proc_1;
+    case HG_UUX_EPEMG: return &hg_proc_2;
+    case HG_UDX_EPVEGG: return &hg_proc_3;
+    case HG_GG_TTXG_DILEP: return &hg_proc_4;
+    case HG_UDX_EPVEGGG: return &hg_proc_5;
+  }
+  return nullptr;
+}
+
+static std::string g_create_error;
+
+}  // namespace hg
+
+struct hg_ctx {
+  int device = 0;
+  int n_sm = 0;
+  bool params_set = false;
+  hg_params par;
+  hg_cuts cuts[HG_N_PROCESS + 1];
+  bool cuts_user = false;
+  hg::Coup<double> coup;
+  double* d_partials = nullptr;  // [kMaxPartialBlocks][3]
+  double* d_acc = nullptr;       // [3]
+  double* h_acc = nullptr;       // pinned [3]
+  void* d_stage = nullptr;       // staging for hg_matrix_element_host
+  size_t stage_bytes = 0;
+  std::string err;
+};
+
+namespace hg {
+
+static int fail(hg_ctx* ctx, int code, const char* msg) {
+  if (ctx) ctx->err = msg;
+  return code;
+}
+static int fail_cuda(hg_ctx* ctx, cudaError_t e, const char* where) {
+  if (ctx) ctx->err = std::string(where) + ": " + cudaGetErrorString(e);
+  return HG_ECUDA;
+}
+
+// Sums nb x 3 partials in a fixed order (deterministic result for a given grid).
+__global__ void finalize_kernel(const double* __restrict__ partials, int nb, double* __restrict__ acc) {
+  __shared__ double sh[3][256];
+  double a = 0, b = 0, c = 0;
+  for (int i = threadIdx.x; i < nb; i += blockDim.x) {
+    a += partials[3 * i];
+    b += partials[3 * i + 1];
+    c += partials[3 * i + 2];
+  }
+  sh[0][threadIdx.x] = a;
+  sh[1][threadIdx.x] = b;
+  sh[2][threadIdx.x] = c;
+  __syncthreads();
+  for (int s = blockDim.x / 2; s > 0; s >>= 1) {
+    if ((int)threadIdx.x < s) {
+      sh[0][threadIdx.x] += sh[0][threadIdx.x + s];
+      sh[1][threadIdx.x] += sh[1][threadIdx.x + s];
+      sh[2][threadIdx.x] += sh[2][threadIdx.x + s];
+    }
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) {
+    acc[0] = sh[0][0];
+    acc[1] = sh[1][0];
+    acc[2] = sh[2][0];
+  }
+}
+
+// Steps a9-a10 on arrays: w = pass * me2 * wps * wscale.
+template <class T>
+__global__ void __launch_bounds__(256) accumulate_kernel(const T* __restrict__ me2, const T* __restrict__ wps,
+                                                         const uint8_t* __restrict__ pass, int64_t n,
+                                                         double wscale, double* __restrict__ partials) {
+  __shared__ double sh[3][8];
+  double sw = 0, sw2 = 0, np = 0;
+  const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+  for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < n; e += stride) {
+    const bool ok = pass ? pass[e] != 0 : true;
+    if (ok) {
+      const double w = (double)me2[e] * (double)wps[e] * wscale;
+      sw += w;
+      sw2 += w * w;
+      np += 1.0;
+    }
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    sw += __shfl_down_sync(0xffffffffu, sw, o);
+    sw2 += __shfl_down_sync(0xffffffffu, sw2, o);
+    np += __shfl_down_sync(0xffffffffu, np, o);
+  }
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  if (lane == 0) {
+    sh[0][w] = sw;
+    sh[1][w] = sw2;
+    sh[2][w] = np;
+  }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double a = 0, b = 0, c = 0;
+    for (int i = 0; i < 8; ++i) {
+      a += sh[0][i];
+      b += sh[1][i];
+      c += sh[2][i];
+    }
+    partials[3 * blockIdx.x] = a;
+    partials[3 * blockIdx.x + 1] = b;
+    partials[3 * blockIdx.x + 2] = c;
+  }
+}
+
+// Register-resident FMA chains: 8 independent accumulators per thread, `iters` x 8 FMAs each.
+template <class T>
+__global__ void __launch_bounds__(256) fma_peak_kernel(T* out, int iters, T a, T b) {
+  T x0 = T(threadIdx.x) * T(1e-3), x1 = x0 + T(1), x2 = x0 + T(2), x3 = x0 + T(3), x4 = x0 + T(4),
+    x5 = x0 + T(5), x6 = x0 + T(6), x7 = x0 + T(7);
+  for (int i = 0; i < iters; ++i) {
+#pragma unroll
+    for (int r = 0; r < 8; ++r) {
+      x0 = x0 * a + b;
+      x1 = x1 * a + b;
+      x2 = x2 * a + b;
+      x3 = x3 * a + b;
+      x4 = x4 * a + b;
+      x5 = x5 * a + b;
+      x6 = x6 * a + b;
+      x7 = x7 * a + b;
+    }
+  }
+  out[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = ((x0 + x1) + (x2 + x3)) + ((x4 + x5) + (x6 + x7));
+}
+
+static bool finite_pos(double x) { return isfinite(x) && x > 0.0; }
+static bool finite_nonneg(double x) { return isfinite(x) && x >= 0.0; }
+
+}  // namespace hg
+
+using namespace hg;
+
+extern "C" {
+
+int hg_create(hg_ctx** out, int cuda_device) {
+  if (!out) {
+    g_create_error = "hg_create: out is NULL";
+    return HG_EINVAL;
+  }
+  *out = nullptr;
+  cudaError_t e = cudaSetDevice(cuda_device);
+  if (e != cudaSuccess) {
+    g_create_error = std::string("hg_create: cudaSetDevice: ") + cudaGetErrorString(e);
+    return HG_ECUDA;
+  }
+  hg_ctx* ctx = new hg_ctx();
+  ctx->device = cuda_device;
+  cudaDeviceProp prop;
+  e = cudaGetDeviceProperties(&prop, cuda_device);
+  if (e == cudaSuccess) e = cudaMalloc(&ctx->d_partials, sizeof(double) * 3 * kMaxPartialBlocks);
+  if (e == cudaSuccess) e = cudaMalloc(&ctx->d_acc, sizeof(double) * 3);
+  if (e == cudaSuccess) e = cudaMallocHost(&ctx->h_acc, sizeof(double) * 3);
+  if (e != cudaSuccess) {
+    g_create_error = std::string("hg_create: ") + cudaGetErrorString(e);
+    hg_destroy(ctx);
+    return HG_ECUDA;
+  }
+  ctx->n_sm = prop.multiProcessorCount;
+  for (int p = 1; p <= HG_N_PROCESS; ++p) default_cuts(p, &ctx->cuts[p]);
+  *out = ctx;
+  return HG_OK;
+}
+
+void hg_destroy(hg_ctx* ctx) {
+  if (!ctx) return;
+  if (ctx->d_partials) cudaFree(ctx->d_partials);
+  if (ctx->d_acc) cudaFree(ctx->d_acc);
+  if (ctx->h_acc) cudaFreeHost(ctx->h_acc);
+  if (ctx->d_stage) cudaFree(ctx->d_stage);
+  delete ctx;
+}
+
+const char* hg_last_error(const hg_ctx* ctx) { return ctx ? ctx->err.c_str() : g_create_error.c_str(); }
+
+void hg_default_params(hg_params* out) {
+  if (out) default_params(out);
+}
+
+int hg_default_cuts(int process, hg_cuts* out) {
+  if (!out) return HG_EINVAL;
+  return default_cuts(process, out) ? HG_OK : HG_ENOPROC;
+}
+
+int hg_process_info(int process, hg_process_info_t* out) {
+  if (!out) return HG_EINVAL;
+  const ProcVTable* vt = vtable(process);
+  if (!vt) return HG_ENOPROC;
+  *out = vt->info;
+  return HG_OK;
+}
+
+int hg_set_params(hg_ctx* ctx, const hg_params* par, const hg_cuts* cuts) {
+  if (!ctx) return HG_EINVAL;
+  if (!par) return fail(ctx, HG_EINVAL, "hg_set_params: par is NULL");
+  if (!finite_pos(par->mz) || !finite_pos(par->mw) || !finite_pos(par->mt) || !finite_pos(par->alpha_em_inv) ||
+      !finite_pos(par->alpha_s) || !finite_pos(par->mh))
+    return fail(ctx, HG_EINVAL, "hg_set_params: masses and couplings must be finite and positive");
+  if (!finite_pos(par->gz) || !finite_pos(par->gw) || !finite_pos(par->gt) || !finite_nonneg(par->gh))
+    return fail(ctx, HG_EINVAL, "hg_set_params: widths must be finite and positive (Breit-Wigner mapping)");
+  if (!finite_nonneg(par->mb)) return fail(ctx, HG_EINVAL, "hg_set_params: mb must be finite and >= 0");
+  if (par->mb != 0.0) return fail(ctx, HG_EINVAL, "hg_set_params: only mb = 0 is generated (BASELINE.json)");
+  if (!(par->mw < par->mz)) return fail(ctx, HG_EINVAL, "hg_set_params: need mw < mz (sw2 = 1 - mw^2/mz^2)");
+  if (par->ckm_diagonal != 1) return fail(ctx, HG_EINVAL, "hg_set_params: only the diagonal CKM is implemented");
+  if (cuts) {
+    const double v[4] = {cuts->pt_jet_min, cuts->eta_jet_max, cuts->eta_lep_max, cuts->dr_jj_min};
+    for (int i = 0; i < 4; ++i)
+      if (!isfinite(v[i])) return fail(ctx, HG_EINVAL, "hg_set_params: cut values must be finite");
+  }
+  ctx->par = *par;
+  ctx->coup = derive_couplings(*par);
+  for (int p = 1; p <= HG_N_PROCESS; ++p) {
+    if (cuts)
+      ctx->cuts[p] = *cuts;
+    else
+      default_cuts(p, &ctx->cuts[p]);
+  }
+  ctx->params_set = true;
+  return HG_OK;
+}
+
+// common argument checks; returns the vtable or NULL (code in *rc)
+static const ProcVTable* check(hg_ctx* ctx, int process, int precision, int64_t n, int* rc, const char* who) {
+  *rc = HG_OK;
+  if (!ctx) {
+    *rc = HG_EINVAL;
+    return nullptr;
+  }
+  const ProcVTable* vt = vtable(process);
+  if (!vt) {
+    *rc = fail(ctx, HG_ENOPROC, (std::string(who) + ": unknown process id").c_str());
+    return nullptr;
+  }
+  if (precision != HG_F64 && precision != HG_F32) {
+    *rc = fail(ctx, HG_EINVAL, (std::string(who) + ": unknown precision").c_str());
+    return nullptr;
+  }
+  if (n < 0) {
+    *rc = fail(ctx, HG_EINVAL, (std::string(who) + ": n < 0").c_str());
+    return nullptr;
+  }
+  if (!ctx->params_set) {
+    *rc = fail(ctx, HG_ENOTSET, (std::string(who) + ": hg_set_params has not been called").c_str());
+    return nullptr;
+  }
+  return vt;
+}
+
+static int check_rs(hg_ctx* ctx, const ProcVTable* vt, int process, double rs, const char* who) {
+  if (!finite_pos(rs)) return fail(ctx, HG_EINVAL, (std::string(who) + ": sqrt_s_hat must be finite and > 0").c_str());
+  if (process == HG_GG_TTXG_DILEP) {
+    // the Breit-Wigner windows must always be kinematically open (reading A14): no rejection on the device
+    const double mtmax = sqrt(ctx->par.mt * ctx->par.mt + ctx->par.mt * ctx->par.gt * fmin(20.0, ctx->par.mt / ctx->par.gt));
+    const double mwmax = sqrt(ctx->par.mw * ctx->par.mw + ctx->par.mw * ctx->par.gw * fmin(20.0, ctx->par.mw / ctx->par.gw));
+    const double mtmin2 = ctx->par.mt * ctx->par.mt - ctx->par.mt * ctx->par.gt * fmin(20.0, ctx->par.mt / ctx->par.gt);
+    if (!(2.0 * mtmax < rs) || !(mtmin2 > 0) || !(mwmax < sqrt(mtmin2)))
+      return fail(ctx, HG_EINVAL, (std::string(who) + ": Breit-Wigner windows not open at this sqrt_s_hat").c_str());
+  }
+  (void)vt;
+  return HG_OK;
+}
+
+int hg_gen_phase_space(hg_ctx* ctx, int process, int precision, uint64_t seed, uint64_t first_event, int64_t n,
+                       double sqrt_s_hat, void* d_p, void* d_wps, uint8_t* d_pass, void* cuda_stream) {
+  int rc;
+  const ProcVTable* vt = check(ctx, process, precision, n, &rc, "hg_gen_phase_space");
+  if (!vt) return rc;
+  if ((rc = check_rs(ctx, vt, process, sqrt_s_hat, "hg_gen_phase_space")) != HG_OK) return rc;
+  if (n == 0) return HG_OK;
+  if (!d_p || !d_wps) return fail(ctx, HG_EINVAL, "hg_gen_phase_space: d_p / d_wps is NULL");
+  const int n_rambo = process == HG_GG_TTXG_DILEP ? 3 : vt->info.n_final;
+  const PsConst k = make_psconst(ctx->par, ctx->cuts[process], n_rambo, sqrt_s_hat);
+  cudaError_t e = vt->ps(precision, n, k, seed, first_event, d_p, d_wps, d_pass, (cudaStream_t)cuda_stream);
+  if (e != cudaSuccess) return fail_cuda(ctx, e, "hg_gen_phase_space");
+  return HG_OK;
+}
+
+int hg_matrix_element(hg_ctx* ctx, int process, int precision, int64_t n, const void* d_p, void* d_me2,
+                      void* cuda_stream) {
+  int rc;
+  const ProcVTable* vt = check(ctx, process, precision, n, &rc, "hg_matrix_element");
+  if (!vt) return rc;
+  if (n == 0) return HG_OK;
+  if (!d_p || !d_me2) return fail(ctx, HG_EINVAL, "hg_matrix_element: d_p / d_me2 is NULL");
+  const size_t al = precision == HG_F64 ? 8 : 4;
+  if (((uintptr_t)d_p % al) || ((uintptr_t)d_me2 % al))
+    return fail(ctx, HG_EINVAL, "hg_matrix_element: misaligned pointer");
+  cudaError_t e = vt->me(precision, n, d_p, d_me2, ctx->coup, (cudaStream_t)cuda_stream);
+  if (e != cudaSuccess) return fail_cuda(ctx, e, "hg_matrix_element");
+  return HG_OK;
+}
+
+int hg_matrix_element_host(hg_ctx* ctx, int process, int precision, int64_t n, const void* h_p, void* h_me2,
+                           void* cuda_stream) {
+  int rc;
+  const ProcVTable* vt = check(ctx, process, precision, n, &rc, "hg_matrix_element_host");
+  if (!vt) return rc;
+  if (n == 0) return HG_OK;
+  if (!h_p || !h_me2) return fail(ctx, HG_EINVAL, "hg_matrix_element_host: h_p / h_me2 is NULL");
+  const size_t el = precision == HG_F64 ? 8 : 4;
+  const size_t in_bytes = el * 4 * (size_t)vt->info.n_ext * (size_t)n, out_bytes = el * (size_t)n;
+  if (ctx->stage_bytes < in_bytes + out_bytes) {
+    if (ctx->d_stage) cudaFree(ctx->d_stage);
+    ctx->d_stage = nullptr;
+    ctx->stage_bytes = 0;
+    cudaError_t e = cudaMalloc(&ctx->d_stage, in_bytes + out_bytes);
+    if (e != cudaSuccess) return fail_cuda(ctx, e, "hg_matrix_element_host: cudaMalloc");
+    ctx->stage_bytes = in_bytes + out_bytes;
+  }
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  char* d_in = (char*)ctx->d_stage;
+  char* d_out = d_in + in_bytes;
+  cudaError_t e = cudaMemcpyAsync(d_in, h_p, in_bytes, cudaMemcpyHostToDevice, s);
+  if (e == cudaSuccess) e = vt->me(precision, n, d_in, d_out, ctx->coup, s);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(h_me2, d_out, out_bytes, cudaMemcpyDeviceToHost, s);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+  if (e != cudaSuccess) return fail_cuda(ctx, e, "hg_matrix_element_host");
+  return HG_OK;
+}
+
+// finalize partials -> acc (host), synchronising the stream
+static int finish(hg_ctx* ctx, int nblocks, int64_t n, double acc[4], cudaStream_t s, const char* who) {
+  finalize_kernel<<<1, 256, 0, s>>>(ctx->d_partials, nblocks, ctx->d_acc);
+  cudaError_t e = cudaGetLastError();
+  if (e == cudaSuccess) e = cudaMemcpyAsync(ctx->h_acc, ctx->d_acc, 3 * sizeof(double), cudaMemcpyDeviceToHost, s);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+  if (e != cudaSuccess) return fail_cuda(ctx, e, who);
+  acc[0] = ctx->h_acc[0];
+  acc[1] = ctx->h_acc[1];
+  acc[2] = (double)n;
+  acc[3] = ctx->h_acc[2];
+  return HG_OK;
+}
+
+int hg_accumulate(hg_ctx* ctx, int precision, int64_t n, const void* d_me2, const void* d_wps,
+                  const uint8_t* d_pass, double sqrt_s_hat, double acc[4], void* cuda_stream) {
+  if (!ctx) return HG_EINVAL;
+  if (precision != HG_F64 && precision != HG_F32) return fail(ctx, HG_EINVAL, "hg_accumulate: unknown precision");
+  if (n < 0) return fail(ctx, HG_EINVAL, "hg_accumulate: n < 0");
+  if (!acc) return fail(ctx, HG_EINVAL, "hg_accumulate: acc is NULL");
+  if (!finite_pos(sqrt_s_hat)) return fail(ctx, HG_EINVAL, "hg_accumulate: sqrt_s_hat must be finite and > 0");
+  acc[0] = acc[1] = acc[2] = acc[3] = 0.0;
+  if (n == 0) return HG_OK;
+  if (!d_me2 || !d_wps) return fail(ctx, HG_EINVAL, "hg_accumulate: d_me2 / d_wps is NULL");
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  const double wscale = kHbarC2Pb / (2.0 * sqrt_s_hat * sqrt_s_hat);
+  int nblocks = ctx->n_sm * 8;
+  if (nblocks > kMaxPartialBlocks) nblocks = kMaxPartialBlocks;
+  const int64_t need = (n + 255) / 256;
+  if (need < nblocks) nblocks = (int)need;
+  if (precision == HG_F64)
+    accumulate_kernel<double><<<nblocks, 256, 0, s>>>((const double*)d_me2, (const double*)d_wps, d_pass, n, wscale,
+                                                      ctx->d_partials);
+  else
+    accumulate_kernel<float><<<nblocks, 256, 0, s>>>((const float*)d_me2, (const float*)d_wps, d_pass, n, wscale,
+                                                     ctx->d_partials);
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return fail_cuda(ctx, e, "hg_accumulate");
+  return finish(ctx, nblocks, n, acc, s, "hg_accumulate");
+}
+
+int hg_integrate_step(hg_ctx* ctx, int process, int precision, uint64_t seed, uint64_t first_event, int64_t n,
+                      double sqrt_s_hat, double acc[4], void* cuda_stream) {
+  int rc;
+  const ProcVTable* vt = check(ctx, process, precision, n, &rc, "hg_integrate_step");
+  if (!vt) return rc;
+  if (!acc) return fail(ctx, HG_EINVAL, "hg_integrate_step: acc is NULL");
+  if ((rc = check_rs(ctx, vt, process, sqrt_s_hat, "hg_integrate_step")) != HG_OK) return rc;
+  acc[0] = acc[1] = acc[2] = acc[3] = 0.0;
+  if (n == 0) return HG_OK;
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  const int n_rambo = process == HG_GG_TTXG_DILEP ? 3 : vt->info.n_final;
+  const PsConst k = make_psconst(ctx->par, ctx->cuts[process], n_rambo, sqrt_s_hat);
+  const double wscale = kHbarC2Pb / (2.0 * sqrt_s_hat * sqrt_s_hat);
+  int per_sm = 1;
+  cudaError_t e = vt->int_blocks_per_sm(precision, &per_sm);
+  if (e != cudaSuccess) return fail_cuda(ctx, e, "hg_integrate_step: occupancy query");
+  if (per_sm < 1) per_sm = 1;
+  int nblocks = ctx->n_sm * per_sm;  // persistent grid: a whole number of resident waves
+  if (nblocks > kMaxPartialBlocks) nblocks = kMaxPartialBlocks;
+  const int64_t need = (n + kIntThreads - 1) / kIntThreads;
+  if (need < nblocks) nblocks = (int)need;
+  e = vt->integrate(precision, n, k, seed, first_event, ctx->coup, wscale, ctx->d_partials, nblocks, s);
+  if (e != cudaSuccess) return fail_cuda(ctx, e, "hg_integrate_step");
+  return finish(ctx, nblocks, n, acc, s, "hg_integrate_step");
+}
+
+int hg_measure_fma_peak(hg_ctx* ctx, int precision, double* flops_per_s, void* cuda_stream) {
+  if (!ctx) return HG_EINVAL;
+  if (!flops_per_s) return fail(ctx, HG_EINVAL, "hg_measure_fma_peak: flops_per_s is NULL");
+  if (precision != HG_F64 && precision != HG_F32) return fail(ctx, HG_EINVAL, "hg_measure_fma_peak: unknown precision");
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  const int blocks = ctx->n_sm * 8, threads = 256, iters = precision == HG_F64 ? 4096 : 8192;
+  void* d_out = nullptr;
+  cudaError_t e = cudaMalloc(&d_out, (size_t)blocks * threads * 8);
+  if (e != cudaSuccess) return fail_cuda(ctx, e, "hg_measure_fma_peak: cudaMalloc");
+  cudaEvent_t e0, e1;
+  cudaEventCreate(&e0);
+  cudaEventCreate(&e1);
+  float best = 1e30f;
+  for (int rep = 0; rep < 6 && e == cudaSuccess; ++rep) {
+    cudaEventRecord(e0, s);
+    if (precision == HG_F64)
+      fma_peak_kernel<double><<<blocks, threads, 0, s>>>((double*)d_out, iters, 0.999999, 1e-6);
+    else
+      fma_peak_kernel<float><<<blocks, threads, 0, s>>>((float*)d_out, iters, 0.99999f, 1e-5f);
+    cudaEventRecord(e1, s);
+    e = cudaEventSynchronize(e1);
+    float ms = 0;
+    if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, e0, e1);
+    if (rep > 0 && ms < best) best = ms;
+  }
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  cudaFree(d_out);
+  if (e != cudaSuccess) return fail_cuda(ctx, e, "hg_measure_fma_peak");
+  const double flops = 2.0 * 64.0 * (double)iters * (double)blocks * (double)threads;
+  *flops_per_s = flops / ((double)best * 1e-3);
+  return HG_OK;
+}
+
+}  // extern "C"

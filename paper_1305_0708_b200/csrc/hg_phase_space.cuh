@@ -1,0 +1,251 @@
+// hg_phase_space.cuh -- on-device phase-space generation, weights and cuts (steps a1-a4).
+//
+// The paper states the problem as: one phase-space point per thread from that thread's random numbers, no
+// rejection loop ("each thread has one chance"), a point that violates a cut gets a null
+// weight, heavy resonances are factorised, dPhi = dPhi_prod prod_k ds_k/2pi dPhi(R_k -> f_k)
+// (Eq. 25-26), with the Breit-Wigner map s = m^2 + m Gamma tan(theta) (Eq. 27,
+// PAPER.md:384-386; A.13-A.15).  BASELINE.json fixes sqrt(s_hat) and asks for flat RAMBO
+// instead of the paper's (y, pT, phi) parameterisation (reading SURVEY.md 8c-A16; draw layout and the
+// constraint-surface projection A16b in DESIGN.md).
+//
+// Everything here is fp64 regardless of the precision of the matrix element: the conformal RAMBO map is
+// ill-conditioned for nearly collinear q_i, and the cut decisions must not depend on the ME precision
+// (reading A17: the fp32 matrix element consumes fp64 momenta rounded to fp32).
+#pragma once
+#include "hg_philox.cuh"
+
+namespace hg {
+
+#define HG_TWO_PI 6.283185307179586476925286766559
+
+HG_HD void hsincos(double x, double& s, double& c) {
+#if defined(__CUDA_ARCH__)
+  sincos(x, &s, &c);
+#else
+  s = sin(x);
+  c = cos(x);
+#endif
+}
+
+// Constants of one hg_gen_phase_space / hg_integrate_step call, prepared on the host.
+struct PsConst {
+  double rs;       // sqrt(s_hat)
+  double vol;      // massless RAMBO volume V_n (constant weight)
+  double mt, mgt;  // top: mass, mass*width
+  double mw, mgw;  // W
+  double mb2;      // m_b^2
+  double tmax_t, tmax_w;  // atan(min(20, m/Gamma))  (A.15; reading A14)
+  double pt_jet_min, eta_jet_max, eta_lep_max, dr_jj_min;  // cuts, <= 0 disables
+};
+
+// isotropic massless momentum of energy e
+HG_HD Mom<double> iso(double uc, double uf, double e) {
+  double c = 2.0 * uc - 1.0;
+  double st = sqrt(1.0 - c * c);
+  double sf, cf;
+  hsincos(HG_TWO_PI * uf, sf, cf);
+  return mkmom<double>(e, e * st * cf, e * st * sf, e * c);
+}
+
+// Flat RAMBO for N massless momenta with total (rs, 0): u[4i..4i+3] = (cos theta, phi, energy, energy) of
+// q_i; conformal map to the rest frame and scale; then the projection A16b.  The weight is the constant V_N.
+template <int N>
+HG_HD void rambo_massless(const double* u, double rs, Mom<double>* p) {
+  Mom<double> Q = mkmom<double>(0, 0, 0, 0);
+#pragma unroll
+  for (int i = 0; i < N; ++i) {
+    p[i] = iso(u[4 * i], u[4 * i + 1], -log(u[4 * i + 2] * u[4 * i + 3]));
+    Q = Q + p[i];
+  }
+  const double rM = 1.0 / sqrt(mdot(Q, Q));
+  const double bx = -Q.x * rM, by = -Q.y * rM, bz = -Q.z * rM;
+  const double x = rs * rM, g = Q.e * rM, a = 1.0 / (1.0 + g);
+  double sx = 0, sy = 0, sz = 0;
+#pragma unroll
+  for (int i = 0; i < N; ++i) {
+    const Mom<double> q = p[i];
+    const double bq = bx * q.x + by * q.y + bz * q.z;
+    const double f = q.e + a * bq;
+    if (i < N - 1) {
+      p[i].x = x * (q.x + bx * f);
+      p[i].y = x * (q.y + by * f);
+      p[i].z = x * (q.z + bz * f);
+      sx += p[i].x;
+      sy += p[i].y;
+      sz += p[i].z;
+    } else {  // A16b: the last 3-momentum closes the sum
+      p[i].x = -sx;
+      p[i].y = -sy;
+      p[i].z = -sz;
+    }
+  }
+  double esum = 0;
+#pragma unroll
+  for (int i = 0; i < N; ++i) {
+    p[i].e = sqrt(p[i].x * p[i].x + p[i].y * p[i].y + p[i].z * p[i].z);
+    esum += p[i].e;
+  }
+  const double lam = rs / esum;
+#pragma unroll
+  for (int i = 0; i < N; ++i) {
+    p[i].e *= lam;
+    p[i].x *= lam;
+    p[i].y *= lam;
+    p[i].z *= lam;
+  }
+}
+
+HG_HD double rambo_volume(int n, double rs) {
+  // V_n = (pi/2)^(n-1) s^(n-2) / ((n-1)! (n-2)!) (2 pi)^(4-3n)
+  double v = 1.0, f1 = 1.0, f2 = 1.0;
+  for (int i = 0; i < n - 1; ++i) v *= 1.5707963267948966;
+  for (int i = 0; i < 2 * n - 4; ++i) v *= rs;
+  for (int i = 2; i <= n - 1; ++i) f1 *= i;
+  for (int i = 2; i <= n - 2; ++i) f2 *= i;
+  v /= f1 * f2;
+  const int e = 3 * n - 4;
+  for (int i = 0; i < e; ++i) v /= HG_TWO_PI;
+  return v;
+}
+
+// Massive RAMBO: rescale the massless 3-momenta by xi with sum_i sqrt(m_i^2 + xi^2 E_i^2) = rs (Newton), and
+// the weight factor (sum|k|/rs)^(2N-3) prod(|k|/E) rs / sum(|k|^2/E)   (reading A16).
+template <int N>
+HG_HD double rambo_massive(const double* u, const double* m2, double msum, double rs, Mom<double>* k) {
+  rambo_massless<N>(u, rs, k);
+  double xi = sqrt(1.0 - (msum / rs) * (msum / rs));
+  for (int it = 0; it < 12; ++it) {
+    double f = -rs, df = 0;
+#pragma unroll
+    for (int i = 0; i < N; ++i) {
+      const double e2 = k[i].e * k[i].e;
+      const double en = sqrt(m2[i] + xi * xi * e2);
+      f += en;
+      df += xi * e2 / en;
+    }
+    xi -= f / df;
+  }
+  double ksum = 0, prod = 1, den = 0;
+#pragma unroll
+  for (int i = 0; i < N; ++i) {
+    const double ka = xi * k[i].e;
+    const double en = sqrt(m2[i] + ka * ka);
+    k[i] = mkmom<double>(en, xi * k[i].x, xi * k[i].y, xi * k[i].z);
+    ksum += ka;
+    prod *= ka / en;
+    den += ka * ka / en;
+  }
+  const double r = ksum / rs;
+  double pw = r;
+  for (int i = 1; i < 2 * N - 3; ++i) pw *= r;
+  return pw * prod * rs / den;
+}
+
+// Eq. 27: s = m^2 + m Gamma tan(theta), theta uniform in +-tmax; returns ds/(2 pi) Jacobian.
+HG_HD double bw_mass(double u, double m, double mg, double tmax, double& s) {
+  const double th = -tmax + 2.0 * tmax * u;
+  s = m * m + mg * tan(th);
+  const double d = s - m * m;
+  return (d * d + mg * mg) / mg * (2.0 * tmax) / HG_TWO_PI;
+}
+
+// pr in the rest frame of P (mass M) -> frame where it moves with P; energy from the mass shell (A16b).
+HG_HD Mom<double> boost_from_rest(const Mom<double>& pr, const Mom<double>& P, double M, double msq) {
+  const double e = (P.e * pr.e + P.x * pr.x + P.y * pr.y + P.z * pr.z) / M;
+  const double fac = (e + pr.e) / (P.e + M);
+  Mom<double> o;
+  o.x = pr.x + fac * P.x;
+  o.y = pr.y + fac * P.y;
+  o.z = pr.z + fac * P.z;
+  o.e = sqrt(o.x * o.x + o.y * o.y + o.z * o.z + msq);
+  return o;
+}
+
+// Isotropic two-body decay P (mass^2 M2) -> (m1sq, m2sq); returns dPhi_2 = |p*| / (4 pi M)  (Eq. 26).
+HG_HD double two_body(const Mom<double>& P, double M2, double m1sq, double m2sq, double uc, double uf,
+                      Mom<double>& p1, Mom<double>& p2) {
+  const double M = sqrt(M2);
+  const double t = M2 - m1sq - m2sq;
+  const double pst = sqrt(t * t - 4.0 * m1sq * m2sq) / (2.0 * M);
+  Mom<double> d = iso(uc, uf, pst);
+  const Mom<double> a = mkmom<double>(sqrt(pst * pst + m1sq), d.x, d.y, d.z);
+  const Mom<double> b = mkmom<double>(sqrt(pst * pst + m2sq), -d.x, -d.y, -d.z);
+  p1 = boost_from_rest(a, P, M, m1sq);
+  p2 = boost_from_rest(b, P, M, m2sq);
+  return pst / (2.0 * HG_TWO_PI * M);
+}
+
+// ---------------------------------------------------------------- per-process generators
+// Writes p[0..n_ext) (leg order of include/hg.h) and returns the phase-space weight.
+template <int NFINAL>
+HG_HD double gen_massless(const PsConst& k, uint64_t seed, uint64_t event, uint32_t pid, Mom<double>* p) {
+  double u[4 * NFINAL];
+  draw_uniforms<4 * NFINAL>(seed, event, pid, u);
+  const double h = 0.5 * k.rs;
+  p[0] = mkmom<double>(h, 0.0, 0.0, h);
+  p[1] = mkmom<double>(h, 0.0, 0.0, -h);
+  rambo_massless<NFINAL>(u, k.rs, p + 2);
+  return k.vol;
+}
+
+// config 4: g g -> (t -> b (W+ -> e+ ve)) (t~ -> b~ (W- -> mu- vm~)) g.  Draws: 0-3 s_t, s_t~, s_W+, s_W-;
+// 4-15 RAMBO(t*, t~*, g); 16,17 t* decay angles; 18,19 W+*; 20,21 t~*; 22,23 W-*.
+HG_HD double gen_ttxg_dilep(const PsConst& k, uint64_t seed, uint64_t event, uint32_t pid, Mom<double>* p) {
+  double u[24];
+  draw_uniforms<24>(seed, event, pid, u);
+  const double h = 0.5 * k.rs;
+  p[0] = mkmom<double>(h, 0.0, 0.0, h);
+  p[1] = mkmom<double>(h, 0.0, 0.0, -h);
+  double st, stb, swp, swm;
+  double w = bw_mass(u[0], k.mt, k.mgt, k.tmax_t, st);
+  w *= bw_mass(u[1], k.mt, k.mgt, k.tmax_t, stb);
+  w *= bw_mass(u[2], k.mw, k.mgw, k.tmax_w, swp);
+  w *= bw_mass(u[3], k.mw, k.mgw, k.tmax_w, swm);
+  const double m2[3] = {st, stb, 0.0};
+  Mom<double> q[3];
+  w *= k.vol * rambo_massive<3>(u + 4, m2, sqrt(st) + sqrt(stb), k.rs, q);
+  Mom<double> wp, wm;
+  w *= two_body(q[0], st, k.mb2, swp, u[16], u[17], p[2], wp);
+  w *= two_body(wp, swp, 0.0, 0.0, u[18], u[19], p[3], p[4]);
+  w *= two_body(q[1], stb, k.mb2, swm, u[20], u[21], p[5], wm);
+  w *= two_body(wm, swm, 0.0, 0.0, u[22], u[23], p[6], p[7]);
+  p[8] = q[2];
+  return w;
+}
+
+// ---------------------------------------------------------------- cuts (Eq. 8-11)
+HG_HD double pt_of(const Mom<double>& p) { return sqrt(p.x * p.x + p.y * p.y); }
+HG_HD double eta_of(const Mom<double>& p) { return asinh(p.z / pt_of(p)); }
+HG_HD double delta_r(const Mom<double>& a, const Mom<double>& b) {  // Eq. 9b
+  const double pi = 0.5 * HG_TWO_PI;
+  double dphi = atan2(a.y, a.x) - atan2(b.y, b.x);
+  if (dphi > pi) dphi -= HG_TWO_PI;
+  if (dphi < -pi) dphi += HG_TWO_PI;
+  const double deta = eta_of(a) - eta_of(b);
+  return sqrt(deta * deta + dphi * dphi);
+}
+
+// P supplies n_jets / jets[] (gluon legs) and n_leps / leps[] (charged leptons) -- scope A11/A12.
+template <class P>
+HG_HD bool passes_cuts(const PsConst& k, const Mom<double>* p) {
+  bool ok = true;
+#pragma unroll
+  for (int a = 0; a < P::n_jets; ++a) {
+    const Mom<double>& j = p[P::jet(a)];
+    if (k.pt_jet_min > 0) ok = ok && (pt_of(j) > k.pt_jet_min);
+    if (k.eta_jet_max > 0) ok = ok && (fabs(eta_of(j)) < k.eta_jet_max);
+  }
+  if (k.eta_lep_max > 0) {
+#pragma unroll
+    for (int a = 0; a < P::n_leps; ++a) ok = ok && (fabs(eta_of(p[P::lep(a)])) < k.eta_lep_max);
+  }
+  if (k.dr_jj_min > 0) {
+#pragma unroll
+    for (int a = 0; a < P::n_jets; ++a)
+#pragma unroll
+      for (int b = a + 1; b < P::n_jets; ++b) ok = ok && (delta_r(p[P::jet(a)], p[P::jet(b)]) > k.dr_jj_min);
+  }
+  return ok;
+}
+
+}  // namespace hg

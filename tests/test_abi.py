@@ -1,0 +1,56 @@
+"""The C-ABI library loads on a CPU-only box and exports every symbol include/hg.h declares; host-only calls work."""
+import os
+import re
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope='module')
+def api():
+    from paper_1305_0708_b200 import build
+    build.build()
+    from paper_1305_0708_b200 import api
+    return api
+
+
+def test_exports_every_declared_symbol(api):
+    hdr = open(os.path.join(ROOT, 'include', 'hg.h')).read()
+    hdr = re.sub(r'/\*.*?\*/', '', hdr, flags=re.S)
+    declared = set(re.findall(r'\b(hg_[a-z0-9_]+)\s*\(', hdr))
+    assert declared == set(api.SYMBOLS)
+    lib = api.load()
+    for s in declared:
+        assert hasattr(lib, s), s
+
+
+def test_process_info_matches_survey_table(api):
+    # SURVEY.md 8a per-config table: (n_ext, hel total / non-zero, diagrams / amplitudes, flows)
+    expect = {1: (4, 16, 1, 1, 1, 1), 2: (5, 32, 8, 4, 4, 1), 3: (6, 64, 4, 8, 8, 2), 4: (9, 512, 8, 16, 18, 6),
+              5: (7, 128, 8, 50, 54, 6)}
+    avg = {1: 1 / 36, 2: 1 / 36, 3: 1 / 72, 4: 1 / 256, 5: 1 / 216}
+    for pid, e in expect.items():
+        i = api.hg_process_info(pid)
+        assert (i['n_ext'], i['n_hel_total'], i['n_hel_nonzero'], i['n_diagrams'], i['n_amplitudes'],
+                i['n_flows']) == e
+        assert abs(i['avg_factor'] - avg[pid]) < 1e-15
+        assert i['flops_f64'] > 100 and i['n_draws'] in (8, 12, 16, 24, 20)
+    with pytest.raises(api.HgError):
+        api.hg_process_info(0)
+
+
+def test_defaults(api):
+    p = api.hg_default_params()
+    assert (p.mz, p.mw, p.gz, p.gw, p.mt, p.gt, p.alpha_em_inv, p.alpha_s) == \
+        (91.1876, 80.419, 2.441, 2.048, 174.3, 1.5, 132.507, 0.118)
+    c = api.hg_default_cuts(5)
+    assert (c.pt_jet_min, c.eta_jet_max, c.eta_lep_max, c.dr_jj_min) == (20.0, 2.5, 0.0, 0.4)
+
+
+def test_no_cpu_fallback(api):
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip('GPU present')
+    with pytest.raises(RuntimeError):
+        api.Context(0)

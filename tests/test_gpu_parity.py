@@ -1,0 +1,282 @@
+"""CUDA path vs oracle, through the C ABI (libhg.so via the ctypes binding), on the same seeded inputs.
+
+Tolerances (BASELINE.json north_star): per-event |Mbar|^2 relative error <= 1e-11 in fp64; fp32 median <= 1e-5 and
+99.9th percentile <= 1e-3 (reading A17: fp32 kernel on fp64 momenta rounded to fp32, error against the oracle at the
+unrounded momenta); integer work (pass flags, counts) exact except where the fp64 cut variable sits within rounding
+of its threshold; cross sections within 3 combined Monte-Carlo standard errors.
+"""
+import math
+
+import numpy as np
+import pytest
+import torch
+
+from oracle import integrate as oint
+from oracle import phase_space as ops
+from oracle import processes as opr
+from oracle import sm as osm
+
+pytestmark = pytest.mark.gpu
+
+PAR = osm.default_params()
+SEED = 13050708
+# events per config for the element-by-element comparison: several 128-thread blocks and a ragged tail, sized so
+# that the oracle finishes in seconds (it costs 15 us .. 50 ms per event)
+N_PARITY = {1: 65536, 2: 4099, 3: 1283, 4: 259, 5: 259}
+
+
+@pytest.fixture(scope='module')
+def ctx():
+    from paper_1305_0708_b200 import api
+    c = api.Context(0)
+    yield c
+    c.close()
+
+
+@pytest.fixture(scope='module')
+def api():
+    from paper_1305_0708_b200 import api
+    return api
+
+
+_ORACLE = {}
+
+
+def oracle_events(cfg):
+    """Oracle momenta, weights, pass flags and |Mbar|^2 of the first N_PARITY events (cached per session)."""
+    if cfg not in _ORACLE:
+        n = N_PARITY[cfg]
+        p, w = ops.generate(cfg, SEED, 0, n, opr.SQRT_S[cfg], PAR)
+        ok = ops.passes(cfg, p)
+        me = opr.me2(opr.config(cfg), p, PAR)
+        _ORACLE[cfg] = (p, w, ok, me)
+    return _ORACLE[cfg]
+
+
+def to_soa(p, dtype):
+    """[n, n_ext, 4] -> device [n_ext, 4, n]."""
+    return torch.from_numpy(np.ascontiguousarray(p.transpose(1, 2, 0))).to(dtype).cuda().contiguous()
+
+
+@pytest.mark.parametrize('cfg', [1, 2, 3, 4, 5])
+def test_matrix_element_fp64(ctx, api, cfg):
+    p, _, _, ref = oracle_events(cfg)
+    got = ctx.hg_matrix_element(cfg, api.HG_F64, to_soa(p, torch.float64)).cpu().numpy()
+    rel = np.abs(got - ref) / ref
+    assert np.all(np.isfinite(got)) and np.all(got > 0)
+    assert rel.max() <= 1e-11, (cfg, rel.max(), int(rel.argmax()))
+
+
+@pytest.mark.parametrize('cfg', [1, 2, 3, 4, 5])
+def test_matrix_element_fp32(ctx, api, cfg):
+    p, _, ok, ref = oracle_events(cfg)
+    got = ctx.hg_matrix_element(cfg, api.HG_F32, to_soa(p, torch.float32)).cpu().numpy().astype(np.float64)
+    sel = ok & (ref > 0)
+    rel = np.abs(got[sel] - ref[sel]) / ref[sel]
+    assert np.all(np.isfinite(got))
+    assert np.median(rel) <= 1e-5, (cfg, np.median(rel))
+    assert np.percentile(rel, 99.9) <= 1e-3, (cfg, np.percentile(rel, 99.9))
+
+
+@pytest.mark.parametrize('cfg', [1, 3])
+def test_matrix_element_host_buffers(ctx, api, cfg):
+    p, _, _, ref = oracle_events(cfg)
+    n = min(len(ref), 1000)
+    hp = torch.from_numpy(np.ascontiguousarray(p[:n].transpose(1, 2, 0))).pin_memory()
+    got = ctx.hg_matrix_element_host(cfg, api.HG_F64, hp).numpy()
+    assert np.max(np.abs(got - ref[:n]) / ref[:n]) <= 1e-11
+
+
+def _rambo_condition(cfg, n):
+    """(Q0/M)^2 of the RAMBO stage: the conformal map amplifies roundings by this factor (A16b)."""
+    from oracle import philox
+    u = philox.uniforms(SEED, 0, n, ops.N_DRAWS[cfg], cfg)
+    if cfg == 4:
+        u, nf = u[:, 4:16], 3
+    else:
+        nf = ops.N_FINAL[cfg]
+    q = np.stack([ops._iso(2 * u[:, 4 * i] - 1, ops.TWO_PI * u[:, 4 * i + 1], -np.log(u[:, 4 * i + 2] * u[:, 4 * i + 3]))
+                  for i in range(nf)], 1)
+    Q = q.sum(1)
+    return Q[:, 0] ** 2 / (Q[:, 0] ** 2 - (Q[:, 1:] ** 2).sum(1))
+
+
+@pytest.mark.parametrize('cfg', [1, 2, 3, 4, 5])
+def test_phase_space_fp64(ctx, api, cfg):
+    p_ref, w_ref, ok_ref, _ = oracle_events(cfg)
+    n = len(w_ref)
+    rs = opr.SQRT_S[cfg]
+    p, w, ok = ctx.hg_gen_phase_space(cfg, api.HG_F64, SEED, 0, n, rs)
+    p = p.cpu().numpy().transpose(2, 0, 1)
+    w = w.cpu().numpy()
+    ok = ok.cpu().numpy().astype(bool)
+    # momenta: both sides evaluate the same formulas in fp64; libm differences (log, sincos, tan) of an ulp or two
+    # are amplified by the conditioning of the conformal map
+    cond = _rambo_condition(cfg, n)
+    tol = 64 * np.finfo(float).eps * rs * np.maximum(cond, 1.0) * (8 if cfg == 4 else 1)
+    dev = np.abs(p - p_ref).reshape(n, -1).max(1)
+    assert np.all(dev <= tol), (cfg, float((dev / tol).max()))
+    assert np.allclose(w, w_ref, rtol=1e-11 if cfg == 4 else 1e-14, atol=0)
+    # the device points satisfy the constraints themselves
+    tot = p[:, 2:].sum(1)
+    assert np.abs(tot - np.array([rs, 0, 0, 0])).max() < 1e-12 * rs
+    # pass flags: identical except where a cut variable is within rounding of its threshold
+    diff = np.nonzero(ok != ok_ref)[0]
+    assert len(diff) <= max(1, n // 10000), (cfg, len(diff))
+
+
+@pytest.mark.parametrize('cfg', [2, 4])
+def test_phase_space_fp32_is_rounded_fp64(ctx, api, cfg):
+    n = 1000
+    rs = opr.SQRT_S[cfg]
+    p64, w64, ok64 = ctx.hg_gen_phase_space(cfg, api.HG_F64, SEED, 0, n, rs)
+    p32, w32, ok32 = ctx.hg_gen_phase_space(cfg, api.HG_F32, SEED, 0, n, rs)
+    assert torch.equal(p64.float(), p32) and torch.equal(w64.float(), w32) and torch.equal(ok64, ok32)
+
+
+def test_phase_space_counter_contract(ctx, api):
+    """Event k uses Philox counter k whatever the batch split (include/hg.h, reading A15)."""
+    cfg, rs = 3, 1000.0
+    p, w, ok = ctx.hg_gen_phase_space(cfg, api.HG_F64, SEED, 0, 700, rs)
+    p2, w2, ok2 = ctx.hg_gen_phase_space(cfg, api.HG_F64, SEED, 300, 400, rs)
+    assert torch.equal(p[:, :, 300:], p2) and torch.equal(w[300:], w2) and torch.equal(ok[300:], ok2)
+    # 64-bit event index: the high word enters the counter
+    p3, _, _ = ctx.hg_gen_phase_space(cfg, api.HG_F64, SEED, (1 << 32) + 300, 4, rs)
+    assert not torch.equal(p3, p2[:, :, :4])
+    pr, _ = ops.generate(cfg, SEED, (1 << 32) + 300, 4, rs, PAR)
+    assert np.allclose(p3.cpu().numpy().transpose(2, 0, 1), pr, rtol=0, atol=1e-9)
+
+
+@pytest.mark.parametrize('cfg', [1, 2, 3, 4, 5])
+@pytest.mark.parametrize('prec', ['f64', 'f32'])
+def test_integrate_step_matches_oracle_weights(ctx, api, cfg, prec):
+    """Fused kernel (a1-a10) against the oracle's per-event weights summed with math.fsum, same events."""
+    p, wps, ok, me = oracle_events(cfg)
+    n = len(me)
+    rs = opr.SQRT_S[cfg]
+    w = me * wps / (2 * rs * rs) * osm.HBARC2_PB * ok
+    ref = oint.accumulate(w, ok)
+    got = ctx.hg_integrate_step(cfg, api.HG_F64 if prec == 'f64' else api.HG_F32, SEED, 0, n, rs)
+    tol = 1e-11 if prec == 'f64' else 2e-5
+    assert got[2] == n
+    assert abs(got[3] - ref[3]) <= max(1, n // 10000)
+    if got[3] == ref[3]:
+        assert abs(got[0] - ref[0]) <= tol * ref[0], (got, ref)
+        assert abs(got[1] - ref[1]) <= 2 * tol * ref[1], (got, ref)
+    # split batches add up (counter contract), independent of the grid
+    a = ctx.hg_integrate_step(cfg, api.HG_F64, SEED, 0, n // 3, rs)
+    b = ctx.hg_integrate_step(cfg, api.HG_F64, SEED, n // 3, n - n // 3, rs)
+    full = ctx.hg_integrate_step(cfg, api.HG_F64, SEED, 0, n, rs)
+    assert abs(a[0] + b[0] - full[0]) <= 1e-12 * full[0] and a[3] + b[3] == full[3]
+
+
+@pytest.mark.parametrize('cfg', [2, 5])
+def test_unfused_path_equals_fused(ctx, api, cfg):
+    """hg_gen_phase_space -> hg_matrix_element -> hg_accumulate gives the sums of hg_integrate_step."""
+    n, rs = 20000, opr.SQRT_S[cfg]
+    p, wps, ok = ctx.hg_gen_phase_space(cfg, api.HG_F64, SEED, 5, n, rs)
+    me = ctx.hg_matrix_element(cfg, api.HG_F64, p)
+    acc = ctx.hg_accumulate(api.HG_F64, me, wps, ok, rs)
+    fused = ctx.hg_integrate_step(cfg, api.HG_F64, SEED, 5, n, rs)
+    assert acc[2] == fused[2] == n and acc[3] == fused[3]
+    assert abs(acc[0] - fused[0]) <= 1e-12 * fused[0] and abs(acc[1] - fused[1]) <= 1e-12 * fused[1]
+    # accumulation against an exact host sum of the device's per-event weights
+    w = (me * wps).cpu().numpy() * ok.cpu().numpy() * osm.HBARC2_PB / (2 * rs * rs)
+    assert abs(acc[0] - math.fsum(w)) <= 1e-12 * math.fsum(w)
+    assert abs(acc[1] - math.fsum(w * w)) <= 1e-12 * math.fsum(w * w)
+    assert acc[3] == int(ok.sum().item())
+
+
+def test_cfg1_cross_section_analytic(ctx, api):
+    """sigma(u d~ -> e+ ve) at sqrt(s)=80 GeV: 7924.94 pb (tests/golden/cfg1_closed_form.txt), full 65,536 events."""
+    acc = ctx.hg_integrate_step(1, api.HG_F64, SEED, 0, 1 << 16, 80.0)
+    s, ds = api.sigma(acc)
+    c = osm.couplings(PAR)
+    shat = 6400.0
+    exact = c['gw'] ** 4 * shat / (576 * math.pi * ((shat - PAR['mw'] ** 2) ** 2 + (PAR['mw'] * PAR['gw']) ** 2)) \
+        * osm.HBARC2_PB
+    assert abs(exact - 7924.94) < 0.01
+    assert abs(s - exact) <= 3 * ds and ds / s < 0.005
+
+
+@pytest.mark.parametrize('cfg', [2, 3, 4, 5])
+def test_full_size_sampled_outputs_and_cross_section(ctx, api, cfg):
+    """BASELINE.json's full sizes in the launch configuration bench.py times: sampled events against the oracle
+    computed one by one, and the cross section against the oracle's subsample within 3 combined standard errors."""
+    n, rs = opr.N_EVENTS[cfg], opr.SQRT_S[cfg]
+    p, wps, ok = ctx.hg_gen_phase_space(cfg, api.HG_F64, SEED, 0, n, rs)
+    me = ctx.hg_matrix_element(cfg, api.HG_F64, p)
+    nsample = {2: 64, 3: 64, 4: 16, 5: 16}[cfg]
+    idx = np.random.default_rng(cfg).integers(0, n, nsample)
+    idx[0], idx[1] = 0, n - 1
+    got = me[torch.from_numpy(idx).cuda()].cpu().numpy()
+    proc = opr.config(cfg)
+    for k, i in enumerate(idx):
+        pr, _ = ops.generate(cfg, SEED, int(i), 1, rs, PAR)
+        ref = opr.me2(proc, pr, PAR)[0]
+        # the device matrix element is evaluated at the device's momenta, which differ from the oracle's by the
+        # conditioning of the RAMBO map (test_phase_space_fp64); compare at the device's own momenta too
+        pd = p[:, :, int(i)].cpu().numpy()[None]
+        ref_d = opr.me2(proc, pd, PAR)[0]
+        assert abs(got[k] - ref_d) <= 1e-11 * ref_d, (cfg, i)
+        assert abs(got[k] - ref) <= 1e-8 * ref, (cfg, i)
+    acc = ctx.hg_integrate_step(cfg, api.HG_F64, SEED, 0, n, rs)
+    s, ds = api.sigma(acc)
+    _, wps_o, ok_o, me_o = oracle_events(cfg)
+    w = me_o * wps_o / (2 * rs * rs) * osm.HBARC2_PB * ok_o
+    so, dso = oint.sigma(oint.accumulate(w, ok_o))
+    assert abs(s - so) <= 3 * math.hypot(ds, dso), (cfg, s, ds, so, dso)
+    acc32 = ctx.hg_integrate_step(cfg, api.HG_F32, SEED, 0, n, rs)
+    s32, ds32 = api.sigma(acc32)
+    assert abs(s32 - s) <= 1e-4 * s and acc32[3] == acc[3]
+
+
+def test_edge_cases_and_errors(ctx, api):
+    from paper_1305_0708_b200.api import HgError
+    # empty batches are successful no-ops
+    assert ctx.hg_integrate_step(3, api.HG_F64, 1, 0, 0, 1000.0) == (0.0, 0.0, 0.0, 0.0)
+    e = torch.empty((6, 4, 0), dtype=torch.float64, device='cuda')
+    assert ctx.hg_matrix_element(3, api.HG_F64, e).numel() == 0
+    # a single event (one partially filled warp)
+    p, w, ok = ctx.hg_gen_phase_space(5, api.HG_F64, 7, 123, 1, 2000.0)
+    me = ctx.hg_matrix_element(5, api.HG_F64, p)
+    ref = opr.me2(opr.config(5), p.cpu().numpy().transpose(2, 0, 1), PAR)
+    assert abs(me.item() - ref[0]) <= 1e-11 * ref[0]
+    with pytest.raises(HgError) as ei:
+        ctx.hg_integrate_step(9, api.HG_F64, 1, 0, 10, 1000.0)
+    assert ei.value.code == api.HG_ENOPROC
+    with pytest.raises(HgError) as ei:
+        ctx.hg_integrate_step(3, 7, 1, 0, 10, 1000.0)
+    assert ei.value.code == api.HG_EINVAL
+    with pytest.raises(HgError) as ei:
+        ctx.hg_integrate_step(3, api.HG_F64, 1, 0, -1, 1000.0)
+    assert ei.value.code == api.HG_EINVAL
+    with pytest.raises(HgError) as ei:
+        ctx.hg_integrate_step(4, api.HG_F64, 1, 0, 10, 300.0)  # below the t t~ Breit-Wigner windows
+    assert ei.value.code == api.HG_EINVAL
+    bad = api.hg_default_params()
+    bad.ckm_diagonal = 0
+    with pytest.raises(HgError):
+        ctx.hg_set_params(bad)
+    ctx.hg_set_params(api.hg_default_params())
+
+
+def test_user_cuts_and_params(ctx, api):
+    """Cuts and SM inputs are run-time parameters: tighter cuts and another alpha_s against the oracle."""
+    cfg, n, rs = 3, 600, 1000.0
+    cuts = api.hg_cuts(50.0, 2.0, 2.0, 0.7)
+    par = api.hg_default_params()
+    par.alpha_s = 0.13
+    ctx.hg_set_params(par, cuts)
+    try:
+        p, wps, ok = ctx.hg_gen_phase_space(cfg, api.HG_F64, SEED, 0, n, rs)
+        me = ctx.hg_matrix_element(cfg, api.HG_F64, p).cpu().numpy()
+    finally:
+        ctx.hg_set_params(api.hg_default_params())
+    po, _ = ops.generate(cfg, SEED, 0, n, rs, PAR)
+    ok_ref = ops.passes(cfg, po, (50.0, 2.0, 2.0, 0.7))
+    assert np.count_nonzero(ok.cpu().numpy().astype(bool) != ok_ref) <= 1
+    assert 0 < ok_ref.sum() < n
+    par_o = dict(PAR, alpha_s=0.13)
+    ref = opr.me2(opr.config(cfg), po[:64], par_o)
+    assert np.max(np.abs(me[:64] - ref) / ref) <= 1e-10
