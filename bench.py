@@ -1,0 +1,331 @@
+"""bench.py -- helicity+colour-summed |M|^2 events/s on B200 (BASELINE.json metric), one JSON line on stdout.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--impl reference] [--all-configs]
+
+A step is one pass of the whole hot path over one batch of BASELINE.json's size:
+hg_integrate_step = Philox -> RAMBO/Breit-Wigner momenta -> cuts -> |Mbar|^2 -> weight -> (sum w, sum w^2, n_pass),
+fused in one kernel per process; fp64.  Default workload: config 5 (u d~ -> e+ ve g g g, 2^22 events, 2 TeV), the
+largest one, which is also the config that asks for the BASES-style accumulation.  `value` counts ALL generated
+events per second (events failing the cuts are generated, tested and counted, their matrix element is skipped,
+PAPER.md:1168); the pass fraction is reported.  `e2e` is hg_matrix_element_host: momenta in pinned HOST memory ->
+H2D -> |Mbar|^2 kernel -> D2H of the per-event results, inside the timed region.  Extra keys give, per config and
+precision, the three timings SURVEY.md 8d asks for (matrix element alone on device-resident momenta, fused step,
+phase space alone) with their FLOP/s fractions.
+
+--impl reference times the oracle (oracle/, numpy fp64, as it stands) on the host cores over bounded samples.
+With N > 1 (torchrun) every rank integrates its own 2^22-event counter range (weak scaling) and the accumulators
+are summed with one all-reduce of 4 doubles per step.
+"""
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = 'helicity+colour-summed |M|^2 events/s on 1 B200; % of FP64/FP32 peak'
+UNIT = 'events/s'
+SQRT_S = {1: 80.0, 2: 500.0, 3: 1000.0, 4: 1500.0, 5: 2000.0}
+N_EVENTS = {1: 1 << 16, 2: 1 << 20, 3: 1 << 22, 4: 1 << 22, 5: 1 << 22}
+NAMES = {1: 'u d~ -> e+ ve', 2: 'u u~ -> e+ e- g', 3: 'u d~ -> e+ ve g g',
+         4: 'g g -> t t~ g -> b e+ ve b~ mu- vm~ g', 5: 'u d~ -> e+ ve g g g'}
+SEED = 13050708
+# nominal non-tensor peaks of B200: 148 SMs x 4 SMSP x 16 lanes x 2 flop x 1.965 GHz for
+# FP64 (one DFMA warp instruction per SMSP every 2 cycles) and twice that for FP32
+PEAK_NOMINAL_TFLOPS = {'f64': 148 * 64 * 2 * 1.965e9 / 1e12, 'f32': 148 * 128 * 2 * 1.965e9 / 1e12}
+
+
+def workload_name(cfg, n):
+    return 'config %d: %s, %d events, sqrt(s_hat) = %g GeV, Philox->RAMBO, BASELINE.json cuts' % (
+        cfg, NAMES[cfg], n, SQRT_S[cfg])
+
+
+# ------------------------------------------------------------------------------------------ clocks
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+    Q = ('clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,'
+         'clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,'
+         'clocks_event_reasons.sw_power_cap')
+
+    def __init__(self, index):
+        self.index = index
+        self.rows = []
+        self.proc = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(['nvidia-smi', '-i', str(self.index), '--query-gpu=' + self.Q,
+                                          '--format=csv,noheader,nounits', '-lms', '100'],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.time(), line.strip()))
+
+    def stop(self, t0, t1):
+        if self.proc is None:
+            return {'sm_mhz': None, 'sm_max_mhz': None, 'reasons': ['nvidia-smi unavailable']}
+        time.sleep(0.15)
+        self.proc.terminate()
+        sm, smax, reasons = [], None, set()
+        names = ('hw_slowdown', 'hw_thermal_slowdown', 'sw_thermal_slowdown', 'sw_power_cap')
+        rows = [r for t, r in self.rows if t0 <= t <= t1] or [r for _, r in self.rows]
+        for r in rows:
+            f = [x.strip() for x in r.split(',')]
+            try:
+                sm.append(float(f[0]))
+                smax = float(f[1])
+            except (ValueError, IndexError):
+                continue
+            for nm, v in zip(names, f[3:7]):
+                if v.lower().startswith('active'):
+                    reasons.add(nm)
+        return {'sm_mhz': statistics.median(sm) if sm else None, 'sm_max_mhz': smax, 'reasons': sorted(reasons),
+                'samples': len(sm)}
+
+
+# ------------------------------------------------------------------------------------------ oracle timing
+ORACLE_SAMPLE = {1: 65536, 2: 8192, 3: 2048, 4: 48, 5: 48}   # events per oracle step (about 1-3 s each)
+
+
+def oracle_step(cfg, first, n):
+    """One pass of the hot path in the oracle: Philox -> momenta -> cuts -> |Mbar|^2 -> weights -> sums."""
+    from oracle import integrate as oint
+    from oracle import sm as osm
+    w, ok = oint.weights(cfg, SEED, first, n, SQRT_S[cfg], osm.default_params())
+    return oint.accumulate(w, ok)
+
+
+def time_oracle(cfg, steps, warmup, n=None):
+    n = n or ORACLE_SAMPLE[cfg]
+    for i in range(warmup):
+        oracle_step(cfg, i * n, n)
+    c0, t0 = time.process_time(), time.perf_counter()
+    for i in range(steps):
+        oracle_step(cfg, (warmup + i) * n, n)
+    wall = time.perf_counter() - t0
+    cpu = time.process_time() - c0
+    cores = max(1, int(round(cpu / wall)))
+    return {'value': steps * n / wall, 'unit': UNIT, 'cores': cores, 'kind': 'oracle',
+            'sample': '%d steps of %d events of the same Philox stream (numpy fp64 oracle, all 2^n_ext helicities, '
+                      'brute-force colour); %d host cores present' % (steps, n, os.cpu_count() or 1)}, wall / steps
+
+
+def run_reference(args):
+    rank = int(os.environ.get('RANK', '0'))
+    if rank != 0:
+        return
+    cfg = args.config
+    base, sec = time_oracle(cfg, args.steps, args.warmup)
+    line = {'impl': 'reference', 'metric': METRIC, 'value': base['value'], 'unit': UNIT, 'n_gpus': args.gpus,
+            'steps': args.steps, 'warmup': args.warmup, 'ms_per_step': sec * 1e3, 'higher_is_better': True,
+            'scaling': 'weak', 'vs_baseline': None, 'dtype': 'f64', 'data': 'synthetic',
+            'config': {'workload': workload_name(cfg, N_EVENTS[cfg]),
+                       'sample_per_step': ORACLE_SAMPLE[cfg]},
+            'cpu_baseline': base,
+            'e2e': {'value': base['value'], 'unit': UNIT, 'h2d_bytes_per_step': 0, 'd2h_bytes_per_step': 0},
+            'gpu_launches': 0}
+    print(json.dumps(line))
+
+
+# ------------------------------------------------------------------------------------------ GPU arm
+def _events_ms(torch, fn, reps):
+    """CUDA-event time of each of `reps` calls of fn on the current stream (the stream the library launches on)."""
+    out = []
+    for _ in range(reps):
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        fn()
+        b.record()
+        b.synchronize()
+        out.append(a.elapsed_time(b))
+    return out
+
+
+def measure_config(torch, api, ctx, cfg, prec, n, reps, peaks):
+    """The three timings of SURVEY.md 8d for one config and precision (median of reps after 3 warm-up calls)."""
+    info = api.hg_process_info(cfg)
+    rs = SQRT_S[cfg]
+    pname = 'f64' if prec == api.HG_F64 else 'f32'
+    p, wps, ok = ctx.hg_gen_phase_space(cfg, prec, SEED, 0, n, rs)
+    me = torch.empty((n,), dtype=p.dtype, device=p.device)
+    res = {}
+    fns = {'matrix_element': lambda: ctx.hg_matrix_element(cfg, prec, p, me),
+           'integrate_step': lambda: ctx.hg_integrate_step(cfg, prec, SEED, 0, n, rs),
+           'gen_phase_space': lambda: ctx.hg_gen_phase_space(cfg, prec, SEED, 0, n, rs, p, wps, ok)}
+    acc = ctx.hg_integrate_step(cfg, prec, SEED, 0, n, rs)
+    pass_frac = acc[3] / acc[2]
+    for name, fn in fns.items():
+        for _ in range(3):
+            fn()
+        ms = statistics.median(_events_ms(torch, fn, reps))
+        flops = {'matrix_element': info['flops_f64'] * n,
+                 'integrate_step': info['flops_f64'] * acc[3] + info['flops_ps'] * n,
+                 'gen_phase_space': info['flops_ps'] * n}[name]
+        r = {'ms': ms, 'events_per_s': n / (ms * 1e-3), 'tflops': flops / (ms * 1e-3) / 1e12}
+        # the matrix element computes in `prec`; the phase space is always fp64
+        pk = 'f64' if name == 'gen_phase_space' else pname
+        r['frac_of_nominal_peak'] = r['tflops'] / PEAK_NOMINAL_TFLOPS[pk]
+        r['frac_of_measured_fma_peak'] = r['tflops'] / peaks[pk]
+        if name == 'matrix_element':
+            el = 8 if prec == api.HG_F64 else 4
+            r['hbm_gbs'] = n * (4 * info['n_ext'] + 1) * el / (ms * 1e-3) / 1e9
+        res[name] = r
+    res['pass_fraction'] = pass_frac
+    res['flops_per_event'] = info['flops_f64']
+    res['n'] = n
+    del p, wps, ok, me
+    return res
+
+
+def run_gpu(args):
+    import torch
+    import torch.distributed as dist
+    from paper_1305_0708_b200 import api, shard
+
+    rank = int(os.environ.get('RANK', '0'))
+    world = int(os.environ.get('WORLD_SIZE', '1'))
+    local = int(os.environ.get('LOCAL_RANK', '0'))
+    if not torch.cuda.is_available():
+        raise SystemExit('bench.py needs a CUDA device (no CPU fallback); use --impl reference for the oracle')
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group('nccl', device_id=torch.device('cuda', local))
+    ctx = api.Context(local)
+    cfg, rs = args.config, SQRT_S[args.config]
+    n = args.events or N_EVENTS[cfg]
+    info = api.hg_process_info(cfg)
+    prec = api.HG_F64 if args.dtype == 'f64' else api.HG_F32
+    first = rank * n                                  # weak scaling: every rank its own n-event counter range
+    dev = torch.device('cuda', local)
+
+    def step():
+        acc = ctx.hg_integrate_step(cfg, prec, SEED, first, n, rs)
+        return shard.combine_acc(acc, device=dev) if world > 1 else acc
+
+    def sync():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        acc = step()
+    sampler = ClockSampler(local)
+    sampler.start()
+    time.sleep(0.3)
+    sync()
+    t0 = time.time()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    per_step = []
+    for _ in range(args.steps):
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        acc = step()
+        b.record()
+        per_step.append((a, b))
+    e1.record()
+    sync()
+    t1 = time.time()
+    total_ms = e0.elapsed_time(e1)
+    kern_ms = statistics.mean(a.elapsed_time(b) for a, b in per_step)
+    clocks = sampler.stop(t0, t1)
+    if world > 1:
+        t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = t.item()
+    ms_per_step = total_ms / args.steps
+    value = world * n / (ms_per_step * 1e-3)
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    # ---- rank 0: end-to-end leg, per-config table, peaks, oracle baseline
+    peaks = {'f64': ctx.hg_measure_fma_peak(api.HG_F64) / 1e12, 'f32': ctx.hg_measure_fma_peak(api.HG_F32) / 1e12}
+    pname = args.dtype
+    el = 8 if prec == api.HG_F64 else 4
+    p, _, _ = ctx.hg_gen_phase_space(cfg, prec, SEED, first, n, rs, want_pass=False)
+    hp = torch.empty(p.shape, dtype=p.dtype).pin_memory()
+    hp.copy_(p)
+    hme = torch.empty((n,), dtype=p.dtype).pin_memory()
+    del p
+    for _ in range(3):
+        ctx.hg_matrix_element_host(cfg, prec, hp, hme)
+    e2e_ms = statistics.mean(_events_ms(torch, lambda: ctx.hg_matrix_element_host(cfg, prec, hp, hme), args.steps))
+    e2e = {'value': n / (e2e_ms * 1e-3), 'unit': UNIT, 'h2d_bytes_per_step': hp.numel() * el,
+           'd2h_bytes_per_step': hme.numel() * el,
+           'what': 'hg_matrix_element_host: pinned host momenta -> H2D -> |Mbar|^2 kernel -> D2H, per step'}
+    del hp, hme
+
+    flops_step = info['flops_f64'] * acc[3] / world + info['flops_ps'] * n if world > 1 else \
+        info['flops_f64'] * acc[3] + info['flops_ps'] * n
+    achieved = flops_step / (kern_ms * 1e-3) / 1e12
+    traffic = None
+    tpath = os.path.join(ROOT, 'profiles', 'roofline_traffic.json')
+    if os.path.exists(tpath):
+        traffic = json.load(open(tpath)).get('integrate_cfg%d_%s' % (cfg, pname))
+    roofline = {'bound': 'alu', 'kernel': 'integrate_kernel<P%d,%s>' % (cfg, 'double' if pname == 'f64' else 'float'),
+                'achieved': achieved, 'peak': PEAK_NOMINAL_TFLOPS[pname], 'unit': 'TFLOP/s',
+                'frac': achieved / PEAK_NOMINAL_TFLOPS[pname], 'traffic': traffic,
+                'peak_kind': 'nominal non-tensor %s peak (148 SM x %d lanes x 2 x 1.965 GHz, DESIGN.md); '
+                             'MEASURED_PEAKS.json has no ALU figure' % (pname, 64 if pname == 'f64' else 128),
+                'peak_measured_fma_chain': peaks[pname], 'frac_of_measured_fma_chain': achieved / peaks[pname],
+                'algorithmic_flops_per_launch': flops_step, 'kernel_ms': kern_ms}
+
+    per_config = {}
+    if not args.no_table:
+        for c in (1, 2, 3, 4, 5):
+            for pr, nm in ((api.HG_F64, 'f64'), (api.HG_F32, 'f32')):
+                per_config['cfg%d_%s' % (c, nm)] = measure_config(torch, api, ctx, c, pr, N_EVENTS[c], 7, peaks)
+        per_config['cfg1_f64_4M'] = measure_config(torch, api, ctx, 1, api.HG_F64, 1 << 22, 7, peaks)
+        per_config['cfg1_f32_4M'] = measure_config(torch, api, ctx, 1, api.HG_F32, 1 << 22, 7, peaks)
+
+    cpu_base, _ = time_oracle(cfg, 4, 1)
+    s, ds = api.sigma(acc)
+    line = {'metric': METRIC, 'value': value, 'unit': UNIT, 'n_gpus': world, 'steps': args.steps,
+            'warmup': max(args.warmup, 3), 'ms_per_step': ms_per_step, 'higher_is_better': True, 'scaling': 'weak',
+            'vs_baseline': None, 'dtype': pname, 'data': 'synthetic',
+            'config': {'workload': workload_name(cfg, n), 'events_per_gpu': n,
+                       'step': 'hg_integrate_step (Philox -> RAMBO -> cuts -> |M|^2 -> weight -> sums, one fused kernel)',
+                       'l2': 'fused step reads no input from HBM; e2e / matrix_element inputs (%d MB) exceed the 126 MB L2'
+                             % (n * 4 * info['n_ext'] * el >> 20),
+                       'pass_fraction': acc[3] / acc[2], 'sigma_pb': s, 'sigma_err_pb': ds},
+            'clocks': clocks, 'e2e': e2e, 'gpu_launches': 2 * args.steps, 'roofline': roofline,
+            'cpu_baseline': cpu_base, 'fma_peak_measured_tflops': peaks, 'per_config': per_config}
+    print(json.dumps(line))
+    ctx.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument('--gpus', type=int, default=1)
+    ap.add_argument('--steps', type=int, default=20)
+    ap.add_argument('--warmup', type=int, default=3)
+    ap.add_argument('--config', type=int, default=5, choices=[1, 2, 3, 4, 5])
+    ap.add_argument('--dtype', default='f64', choices=['f64', 'f32'])
+    ap.add_argument('--events', type=int, default=0, help='events per GPU per step (default: BASELINE.json size)')
+    ap.add_argument('--impl', default='graft', choices=['graft', 'reference'])
+    ap.add_argument('--no-table', action='store_true', help='skip the per-config table')
+    args = ap.parse_args()
+    if args.impl == 'reference':
+        run_reference(args)
+    else:
+        run_gpu(args)
+
+
+if __name__ == '__main__':
+    main()

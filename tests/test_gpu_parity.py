@@ -225,6 +225,13 @@ def test_full_size_sampled_outputs_and_cross_section(ctx, api, cfg):
     _, wps_o, ok_o, me_o = oracle_events(cfg)
     w = me_o * wps_o / (2 * rs * rs) * osm.HBARC2_PB * ok_o
     so, dso = oint.sigma(oint.accumulate(w, ok_o))
+    # The weights are heavy-tailed (soft / collinear enhancement down to the cuts): the sample variance of the
+    # oracle's few-hundred-event subsample underestimates its own error whenever the tail was not hit.  Its
+    # standard error is therefore taken as the larger of its own estimate and sqrt(Var_w / n_sub) with the variance
+    # of the weight distribution measured on the full sample.  (The exact statement -- identical sums on identical
+    # events -- is test_integrate_step_matches_oracle_weights.)
+    var_w = acc[1] / acc[2] - s * s
+    dso = max(dso, math.sqrt(var_w / len(w)))
     assert abs(s - so) <= 3 * math.hypot(ds, dso), (cfg, s, ds, so, dso)
     acc32 = ctx.hg_integrate_step(cfg, api.HG_F32, SEED, 0, n, rs)
     s32, ds32 = api.sigma(acc32)
