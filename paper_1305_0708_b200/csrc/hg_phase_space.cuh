@@ -18,12 +18,15 @@ namespace hg {
 
 #define HG_TWO_PI 6.283185307179586476925286766559
 
-HG_HD void hsincos(double x, double& s, double& c) {
+// sin, cos of 2 pi u.  On the device sincospi(2u): exact argument reduction, so no call to the Payne-Hanek slow path
+// of sincos() is left in the fused kernels (a real CALL inside the W+3 jets fp64 kernel made ptxas fall back to an
+// all-on-stack allocation, profiles/r01_notes.md).
+HG_HD void hsincos2pi(double u, double& s, double& c) {
 #if defined(__CUDA_ARCH__)
-  sincos(x, &s, &c);
+  sincospi(2.0 * u, &s, &c);
 #else
-  s = sin(x);
-  c = cos(x);
+  s = sin(HG_TWO_PI * u);
+  c = cos(HG_TWO_PI * u);
 #endif
 }
 
@@ -43,7 +46,7 @@ HG_HD Mom<double> iso(double uc, double uf, double e) {
   double c = 2.0 * uc - 1.0;
   double st = sqrt(1.0 - c * c);
   double sf, cf;
-  hsincos(HG_TWO_PI * uf, sf, cf);
+  hsincos2pi(uf, sf, cf);
   return mkmom<double>(e, e * st * cf, e * st * sf, e * c);
 }
 
