@@ -436,4 +436,47 @@ HG_HD Vc<T> jgggxx(const Vc<T>& v1, const Vc<T>& v2, const Vc<T>& v3, T g2, D d)
   return w;
 }
 
+// =============================================================================== closing on a massless vector leg
+// The amplitude of a diagram is linear in the wavefunction of its last external leg.  When that leg is a massless
+// vector boson, eps(h) = (0, s Re e + i Im e) with e = eps(+1), s = +1 (h = +1) or -1 (h = -1, vflip), so
+//   amplitude(h) = eps(h).B = -(s rb + i ib),   rb = sum_i Re(e_i) B_i,  ib = sum_i Im(e_i) B_i   (i = 1..3)
+// for the bare current B of the closing vertex (the off-shell functions below without their propagator).  The
+// generator accumulates rb, ib per colour flow once and forms both helicities at the end: the loop over the last
+// helicity and half of the closing arithmetic disappear.
+template <class T>
+HG_HD void close_proj(const Vc<T>& e, const Vc<T>& b, cx<T>& rb, cx<T>& ib) {
+  rb = mk<T>(e.c[1].re * b.c[1].re + e.c[2].re * b.c[2].re + e.c[3].re * b.c[3].re,
+             e.c[1].re * b.c[1].im + e.c[2].re * b.c[2].im + e.c[3].re * b.c[3].im);
+  ib = mk<T>(e.c[1].im * b.c[1].re + e.c[2].im * b.c[2].re + e.c[3].im * b.c[3].re,
+             e.c[1].im * b.c[1].im + e.c[2].im * b.c[2].im + e.c[3].im * b.c[3].im);
+}
+// amplitude for helicity sign s from the accumulated projections
+template <class T>
+HG_HD cx<T> close_amp(cx<T> x, cx<T> y, T s) {
+  return mk<T>(y.im - s * x.re, -(s * x.im) - y.re);
+}
+// bare three-vector current (jvvxxx without propagator):  v3.jvv_bare(v1,v2) = vvvxxx(v1,v2,v3), k3 = -(k1+k2)
+template <class T>
+HG_HD Vc<T> jvv_bare(const Vc<T>& v1, const Vc<T>& v2, T g, const Mom<T>& k1, const Mom<T>& k2) {
+  cx<T> d12 = g * vdot(v1, v2);
+  cx<T> a = g * vdot(k2 + k2 + k1, v1);
+  cx<T> b = g * vdot(k1 + k1 + k2, v2);
+  Mom<T> dk = k1 - k2;
+  Vc<T> j;
+  j.c[0] = cfma(a, v2.c[0], dk.e * d12) - b * v1.c[0];
+  j.c[1] = cfma(a, v2.c[1], dk.x * d12) - b * v1.c[1];
+  j.c[2] = cfma(a, v2.c[2], dk.y * d12) - b * v1.c[2];
+  j.c[3] = cfma(a, v2.c[3], dk.z * d12) - b * v1.c[3];
+  return j;
+}
+// bare four-gluon current of one colour structure:  v4.jggg_bare(v1,v2,v3) = ggggxx(v1,v2,v3,v4)
+template <class T>
+HG_HD Vc<T> jggg_bare(const Vc<T>& v1, const Vc<T>& v2, const Vc<T>& v3, T g2) {
+  cx<T> a = g2 * vdot(v1, v3);
+  cx<T> b = g2 * vdot(v2, v3);
+  Vc<T> w;
+  for (int i = 0; i < 4; ++i) w.c[i] = a * v2.c[i] - b * v1.c[i];
+  return w;
+}
+
 }  // namespace hg

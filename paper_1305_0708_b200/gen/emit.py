@@ -37,6 +37,9 @@ class Emitter:
         self.legs = diag.legs
         self.static = [l.index for l in self.legs if l.particle.spin == 'F' and not l.particle.mass]
         self.dynamic = [l.index for l in self.legs if l.index not in self.static]
+        if diag.last in self.dynamic:      # the closing leg is the innermost one
+            self.dynamic.remove(diag.last)
+            self.dynamic.append(diag.last)
         self.nhel = {}
         for l in self.legs:
             p = l.particle
@@ -313,11 +316,55 @@ class CodeGen(Emitter):
             return 'ggggxx(%s, %s, %s, %s, %s)' % (nm(x), nm(y), nm(z), nm(d4), self._cpl(v.coup[0]))
         raise NotImplementedError(v.kind)
 
+    def closes_by_current(self):
+        """True if the last leg is a massless vector boson: the roots are then evaluated as bare currents projected
+        on eps(+1) of that leg (hg_helas.cuh "closing on a massless vector leg") and its helicity is not looped."""
+        if not self.dynamic or self.dynamic[-1] != self.dg.last:
+            return False
+        p = self.legs[self.dg.last].particle
+        return p.spin == 'V' and not p.mass
+
+    def _root_current_expr(self, rt, vi, hel):
+        v = rt.vertex
+        by_slot = dict(zip(rt.slots, rt.children))
+        nm = lambda ch: self._name(ch, vi, hel)
+        mk = lambda ch: self._node_mask(ch, hel, self.memo)
+        last = self.dg.last
+        is_last = lambda ch: ch.is_leaf and ch.leg == last
+        if v.kind == 'FFV':
+            row, col, vec = by_slot[0], by_slot[1], by_slot[2]
+            assert is_last(vec)
+            return 'ffv_current<%d, %d, %d>(%s, %s, %s, %s)' % (
+                mk(col), mk(row), self._gmask(v), nm(col), nm(row), self._cpl(v.coup[0]), self._cpl(v.coup[1]))
+        if v.kind == 'VVV':
+            (sl,) = [s_ for s_, ch in by_slot.items() if is_last(ch)]
+            a, b = by_slot[(sl + 1) % 3], by_slot[(sl + 2) % 3]
+            return 'jvv_bare(%s, %s, %s, %s, %s)' % (nm(a), nm(b), self._cpl(v.coup[0]), self._K(a.mask),
+                                                     self._K(b.mask))
+        if v.kind == 'VVVV':
+            if v.colour != 'ff':
+                raise NotImplementedError('electroweak four-boson vertex (K13, out of scope)')
+            a, b, c3, d4 = [by_slot[s_] for s_ in sorted(by_slot)]
+            x, y, z = {1: (a, b, c3), 2: (a, c3, b), 3: (b, c3, a)}[rt.struct]
+            # ggggxx(x, y, z, d4) = g2 [(x.z)(y.d4) - (y.z)(x.d4)], solved for the closing leg
+            if is_last(d4):
+                t = (x, y, z)
+            elif is_last(z):
+                t = (y, x, d4)
+            elif is_last(y):
+                t = (z, d4, x)
+            else:
+                assert is_last(x)
+                t = (d4, z, y)
+            return 'jggg_bare(%s, %s, %s, %s)' % (nm(t[0]), nm(t[1]), nm(t[2]), self._cpl(v.coup[0]))
+        raise NotImplementedError(v.kind)
+
     # ------------------------------------------------------------------ one static-helicity variant
     def _emit_variant(self, vi, hel, roots, cmat):
         dyn = self.dynamic
-        k = len(dyn)
-        levels = [[] for _ in range(k + 1)]   # lines per loop depth
+        cbc = self.closes_by_current()
+        k = len(dyn) - 1 if cbc else len(dyn)   # number of helicity loops
+        levels = [[] for _ in range(k + 1)]     # lines per loop depth
         done = set()
 
         def need(nd):
@@ -345,10 +392,24 @@ class CodeGen(Emitter):
         nf = len(self.flows)
         fidx = {w: i for i, w in enumerate(self.flows)}
         inner = levels[k]
-        # order the roots so that diagrams sharing deep sub-currents are adjacent
+        last = self.dg.last
         for rt in roots:
             for ch in rt.children:
                 need(ch)
+            if cbc:
+                inner.append('{ const Vc<T> b = %s;' % self._root_current_expr(rt, vi, hel))
+                inner.append('  cx<T> rb, ib;')
+                inner.append('  close_proj(e%d, b, rb, ib);' % last)
+                for w, cf in sorted(rt.colour.terms.items()):
+                    f = fidx[w]
+                    if cf == 1:
+                        inner.append('  X%d = X%d + rb; Y%d = Y%d + ib;' % (f, f, f, f))
+                    elif cf == -1:
+                        inner.append('  X%d = X%d - rb; Y%d = Y%d - ib;' % (f, f, f, f))
+                    else:
+                        inner.append('  X%d = X%d + T(%d) * rb; Y%d = Y%d + T(%d) * ib;' % (f, f, cf, f, f, cf))
+                inner.append('}')
+                continue
             inner.append('{ const cx<T> a = %s;' % self._root_expr(rt, vi, hel))
             for w, cf in sorted(rt.colour.terms.items()):
                 f = fidx[w]
@@ -361,6 +422,13 @@ class CodeGen(Emitter):
             inner.append('}')
         # colour contraction (symmetric form)
         tail = []
+        if cbc:
+            tail.append('#pragma unroll')
+            tail.append('for (int h%d = 0; h%d < 2; ++h%d) {' % (last, last, last))
+            tail.append('  const T sg = h%d ? T(-1) : T(1);' % last)
+            tail.append('  const cx<T> ' + ', '.join('j%d = close_amp(X%d, Y%d, sg)' % (f, f, f) for f in range(nf))
+                        + ';')
+        pre = '  ' if cbc else ''
         for f in range(nf):
             terms = []
             for g in range(f, nf):
@@ -368,7 +436,13 @@ class CodeGen(Emitter):
                 if cval == 0:
                     continue
                 terms.append('T(%d) * j%d' % (cval, g))
-            tail.append('{ const cx<T> t = %s; me += j%d.re * t.re + j%d.im * t.im; }' % (' + '.join(terms), f, f))
+            tail.append(pre + '{ const cx<T> t = %s; me += j%d.re * t.re + j%d.im * t.im; }' % (
+                ' + '.join(terms), f, f))
+        if cbc:
+            tail.append('}')
+            accdecl = 'cx<T> ' + ', '.join('X%d = czero<T>(), Y%d = czero<T>()' % (f, f) for f in range(nf)) + ';'
+        else:
+            accdecl = 'cx<T> ' + ', '.join('j%d = czero<T>()' % f for f in range(nf)) + ';'
         # assemble
         b = self.body
         ind = '  '
@@ -376,7 +450,7 @@ class CodeGen(Emitter):
                  ', '.join('%s(%d)=%+d' % (self.legs[l].name, l, h) for l, h in sorted(hel.items())))
         ind += '  '
         if k == 0:
-            b.append(ind + 'cx<T> ' + ', '.join('j%d = czero<T>()' % f for f in range(nf)) + ';')
+            b.append(ind + accdecl)
         for line in levels[0]:
             b.append(ind + line)
         for d in range(1, k + 1):
@@ -388,7 +462,7 @@ class CodeGen(Emitter):
             ind += '  '
             b.append(ind + self._dyn_leaf_decl(lg))
             if d == k:
-                b.append(ind + 'cx<T> ' + ', '.join('j%d = czero<T>()' % f for f in range(nf)) + ';')
+                b.append(ind + accdecl)
             for line in levels[d]:
                 b.append(ind + line)
         for line in tail:
