@@ -40,6 +40,8 @@ struct hg_ctx {
   double* h_acc = nullptr;       // pinned [3]
   void* d_stage = nullptr;       // staging for hg_matrix_element_host
   size_t stage_bytes = 0;
+  void* d_scratch = nullptr;     // phase-space points of one chunk of hg_integrate_step (staged processes)
+  size_t scratch_bytes = 0;
   std::string err;
 };
 
@@ -190,6 +192,7 @@ void hg_destroy(hg_ctx* ctx) {
   if (ctx->d_acc) cudaFree(ctx->d_acc);
   if (ctx->h_acc) cudaFreeHost(ctx->h_acc);
   if (ctx->d_stage) cudaFree(ctx->d_stage);
+  if (ctx->d_scratch) cudaFree(ctx->d_scratch);
   delete ctx;
 }
 
@@ -402,7 +405,21 @@ int hg_integrate_step(hg_ctx* ctx, int process, int precision, uint64_t seed, ui
   if (nblocks > kMaxPartialBlocks) nblocks = kMaxPartialBlocks;
   const int64_t need = (n + kIntThreads - 1) / kIntThreads;
   if (need < nblocks) nblocks = (int)need;
-  e = vt->integrate(precision, n, k, seed, first_event, ctx->coup, wscale, ctx->d_partials, nblocks, s);
+  const size_t per_event = vt->scratch_bytes_per_event(precision);
+  const int64_t chunk = n < kIntChunk ? n : kIntChunk;
+  if (per_event) {  // two kernels per chunk through a context-owned buffer, grown on demand
+    const size_t bytes = per_event * (size_t)chunk + 1024;
+    if (bytes > ctx->scratch_bytes) {
+      if (ctx->d_scratch) cudaFree(ctx->d_scratch);
+      ctx->d_scratch = nullptr;
+      ctx->scratch_bytes = 0;
+      e = cudaMalloc(&ctx->d_scratch, bytes);
+      if (e != cudaSuccess) return fail_cuda(ctx, e, "hg_integrate_step: cudaMalloc of the chunk buffer");
+      ctx->scratch_bytes = bytes;
+    }
+  }
+  e = vt->integrate(precision, n, k, seed, first_event, ctx->coup, wscale, ctx->d_partials, nblocks, ctx->d_scratch,
+                    chunk, s);
   if (e != cudaSuccess) return fail_cuda(ctx, e, "hg_integrate_step");
   return finish(ctx, nblocks, n, acc, s, "hg_integrate_step");
 }

@@ -390,6 +390,15 @@ HG_HD Vc<T> jioxxx(const Sp<T>& fi, const Sp<T>& fo, T gL, T gR, const Mom<T>& q
   return vprop<UNITARY>(ffv_current<MI, MO, G>(fi, fo, gL, gR), q, rm2, d);
 }
 
+// massless vector line (Feynman gauge): d J, no momentum needed
+template <int MI, int MO, int G, class T, class D>
+HG_HD Vc<T> jioxx0(const Sp<T>& fi, const Sp<T>& fo, T gL, T gR, D d) {
+  const Vc<T> j = ffv_current<MI, MO, G>(fi, fo, gL, gR);
+  Vc<T> w;
+  for (int i = 0; i < 4; ++i) w.c[i] = d * j.c[i];
+  return w;
+}
+
 // =============================================================================== VVV (Eq. 40-44)
 // vvvxxx: g [ (v1.v2)(k1-k2).v3 + (v2.v3)(k2-k3).v1 + (v3.v1)(k3-k1).v2 ], all momenta incoming
 // (PAPER.md:535-567, 1773-1810).  For gluons the colour factor i f^{abc} is handled by the generator.

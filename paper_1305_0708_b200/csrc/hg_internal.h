@@ -13,6 +13,8 @@ namespace hg {
 // Grid of the fused integrate kernel: persistent, HG_INT_BLOCKS_PER_SM blocks of HG_INT_THREADS per SM.
 constexpr int kIntThreads = 128;
 constexpr int kMaxPartialBlocks = 148 * 16;
+// events per chunk of the two-kernel step of staged processes (the chunk buffer is 233 MB for W + 3 jets, fp64)
+constexpr int64_t kIntChunk = (int64_t)1 << 20;
 
 struct ProcVTable {
   hg_process_info_t info;
@@ -22,11 +24,15 @@ struct ProcVTable {
   cudaError_t (*ps)(int prec, int64_t n, const PsConst& k, uint64_t seed, uint64_t first, void* d_p,
                     void* d_wps, uint8_t* d_pass, cudaStream_t s);
   // hg_integrate_step: writes nblocks x (sum w, sum w^2, n_pass) partials; wscale = (hbar c)^2 / (2 s_hat)
+  // Staged processes (scratch_bytes_per_event > 0) run the step as two kernels per chunk of `chunk` events
+  // through the caller's scratch buffer (momenta, weight, pass flag); the others ignore scratch and chunk.
   cudaError_t (*integrate)(int prec, int64_t n, const PsConst& k, uint64_t seed, uint64_t first,
                            const Coup<double>& c, double wscale, double* d_partials, int nblocks,
-                           cudaStream_t s);
+                           void* d_scratch, int64_t chunk, cudaStream_t s);
   // resident blocks per SM of the fused kernel for this precision (occupancy query)
   cudaError_t (*int_blocks_per_sm)(int prec, int* out);
+  // bytes of scratch per event of a chunk for the given precision (0: the step is one fused kernel)
+  size_t (*scratch_bytes_per_event)(int prec);
 };
 
 extern const ProcVTable hg_proc_1, hg_proc_2, hg_proc_3, hg_proc_4, hg_proc_5;

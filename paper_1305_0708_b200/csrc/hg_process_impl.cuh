@@ -12,24 +12,54 @@
 //     registers, the block reduces (sum w, sum w^2, n_pass) with warp shuffles and writes one partial.
 #pragma once
 #include "hg_internal.h"
+#include "hg_stage.cuh"
 
 namespace hg {
 
+// Threads per block of a kernel that evaluates me2<T>.  A staged process needs P::n_stage words of shared memory
+// per thread, which is what limits the warps resident on an SM (227 KB).  All of them go into one block (two
+// blocks when more than 6 fit) because the warps of a block run the generated code in step (SmemStage::sync).
+constexpr int kSmemPerSM = 227 * 1024;
 template <class P, class T>
-__global__ void __launch_bounds__(P::me_threads) me_kernel(const T* __restrict__ p, T* __restrict__ me2,
-                                                           int64_t n, const Coup<T> c) {
-  const int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (e >= n) return;
+constexpr int stage_threads(int want) {
+  if (P::n_stage == 0) return want;
+  const int fit = kSmemPerSM / (P::n_stage * (int)sizeof(T) * 32);
+  const int w = fit <= 6 ? fit : (fit <= 12 ? fit / 2 : 6);
+  return 32 * (w < 1 ? 1 : w);
+}
+template <class P, class T, int THREADS>
+constexpr size_t stage_bytes() {
+  return (size_t)P::n_stage * sizeof(T) * THREADS;
+}
+
+// me2 of one event with the staging area of this thread (shared memory laid out [slot][thread], hg_stage.cuh)
+template <class P, class T, int THREADS>
+__device__ __forceinline__ T me2_event(const Mom<T>* q, const Coup<T>& c) {
+  if constexpr (P::n_stage > 0) {
+    extern __shared__ __align__(16) unsigned char hg_stage_smem[];
+    const SmemStage<T, THREADS> st{reinterpret_cast<T*>(hg_stage_smem) + threadIdx.x};
+    return P::template me2<T>(q, c, st);
+  } else {
+    return P::template me2<T>(q, c, NoStage{});
+  }
+}
+
+template <class P, class T, int THREADS>
+__global__ void __launch_bounds__(THREADS) me_kernel(const T* __restrict__ p, T* __restrict__ me2, int64_t n,
+                                                     const Coup<T> c) {
+  const int64_t e0 = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const int64_t e = e0 < n ? e0 : n - 1;  // no early exit: a staged me2 holds block-wide rendezvous
   Mom<T> q[P::n_ext];
 #pragma unroll
   for (int l = 0; l < P::n_ext; ++l)
     q[l] = mkmom<T>(p[(l * 4 + 0) * n + e], p[(l * 4 + 1) * n + e], p[(l * 4 + 2) * n + e], p[(l * 4 + 3) * n + e]);
-  me2[e] = P::template me2<T>(q, c);
+  const T r = me2_event<P, T, THREADS>(q, c);
+  if (e0 < n) me2[e0] = r;
 }
 
-template <class P, class T>
+template <class P, class T, class W>
 __global__ void __launch_bounds__(128) ps_kernel(const PsConst k, uint64_t seed, uint64_t first, int64_t n,
-                                                 T* __restrict__ p, T* __restrict__ wps,
+                                                 T* __restrict__ p, W* __restrict__ wps,
                                                  uint8_t* __restrict__ pass) {
   const int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (e >= n) return;
@@ -42,7 +72,7 @@ __global__ void __launch_bounds__(128) ps_kernel(const PsConst k, uint64_t seed,
     p[(l * 4 + 2) * n + e] = T(q[l].y);
     p[(l * 4 + 3) * n + e] = T(q[l].z);
   }
-  wps[e] = T(w);
+  wps[e] = W(w);
   if (pass) pass[e] = passes_cuts<P>(k, q) ? 1 : 0;
 }
 
@@ -75,8 +105,8 @@ __device__ __forceinline__ void block_reduce3(double& a, double& b, double& c) {
   }
 }
 
-template <class P, class T>
-__global__ void __launch_bounds__(kIntThreads) integrate_kernel(const PsConst k, uint64_t seed, uint64_t first,
+template <class P, class T, int THREADS>
+__global__ void __launch_bounds__(THREADS) integrate_kernel(const PsConst k, uint64_t seed, uint64_t first,
                                                                 int64_t n, const Coup<T> c, double wscale,
                                                                 double* __restrict__ partials) {
   double sw = 0.0, sw2 = 0.0, np = 0.0;
@@ -88,7 +118,7 @@ __global__ void __launch_bounds__(kIntThreads) integrate_kernel(const PsConst k,
       Mom<T> qt[P::n_ext];
 #pragma unroll
       for (int l = 0; l < P::n_ext; ++l) qt[l] = mkmom<T>(T(q[l].e), T(q[l].x), T(q[l].y), T(q[l].z));
-      const double w = (double)P::template me2<T>(qt, c) * wps * wscale;
+      const double w = (double)me2_event<P, T, THREADS>(qt, c) * wps * wscale;
       sw += w;
       sw2 += w * w;
       np += 1.0;
@@ -102,39 +132,138 @@ __global__ void __launch_bounds__(kIntThreads) integrate_kernel(const PsConst k,
   }
 }
 
+// Second half of the step of a staged process: reads the points the ps_kernel wrote (momenta as T, weight as
+// double, pass flag), evaluates |M|^2 and reduces (sum w, sum w^2, n_pass) per block.  The two halves are separate
+// kernels because the phase-space code wants ~70 registers at full occupancy while the staged matrix element
+// runs at 5-6 warps per SM; the round trip through HBM is 32 n_ext + 9 bytes per event against >= 2e4 flops.
+// A block skips me2 only if none of its events passes (every thread must reach the rendezvous inside me2).
+template <class P, class T, int THREADS>
+__global__ void __launch_bounds__(THREADS) me_acc_kernel(const T* __restrict__ p, const double* __restrict__ wps,
+                                                         const uint8_t* __restrict__ pass, int64_t n,
+                                                         const Coup<T> c, double wscale, int add,
+                                                         double* __restrict__ partials) {
+  double sw = 0.0, sw2 = 0.0, np = 0.0;
+  for (int64_t base = (int64_t)blockIdx.x * THREADS; base < n; base += (int64_t)gridDim.x * THREADS) {
+    const int64_t e0 = base + threadIdx.x;
+    const int64_t e = e0 < n ? e0 : n - 1;
+    const bool ok = e0 < n && pass[e] != 0;
+    if (__syncthreads_or(ok)) {
+      Mom<T> q[P::n_ext];
+#pragma unroll
+      for (int l = 0; l < P::n_ext; ++l)
+        q[l] = mkmom<T>(p[(l * 4 + 0) * n + e], p[(l * 4 + 1) * n + e], p[(l * 4 + 2) * n + e],
+                        p[(l * 4 + 3) * n + e]);
+      const double w = (double)me2_event<P, T, THREADS>(q, c) * wps[e] * wscale;
+      if (ok) {
+        sw += w;
+        sw2 += w * w;
+        np += 1.0;
+      }
+    }
+  }
+  block_reduce3(sw, sw2, np);
+  if (threadIdx.x == 0) {
+    if (add) {
+      sw += partials[3 * blockIdx.x + 0];
+      sw2 += partials[3 * blockIdx.x + 1];
+      np += partials[3 * blockIdx.x + 2];
+    }
+    partials[3 * blockIdx.x + 0] = sw;
+    partials[3 * blockIdx.x + 1] = sw2;
+    partials[3 * blockIdx.x + 2] = np;
+  }
+}
+
 template <class P>
 struct Launch {
-  static cudaError_t me(int prec, int64_t n, const void* d_p, void* d_me2, const Coup<double>& c, cudaStream_t s) {
-    const unsigned grid = (unsigned)((n + P::me_threads - 1) / P::me_threads);
-    if (prec == HG_F64)
-      me_kernel<P, double><<<grid, P::me_threads, 0, s>>>((const double*)d_p, (double*)d_me2, n, c);
-    else
-      me_kernel<P, float><<<grid, P::me_threads, 0, s>>>((const float*)d_p, (float*)d_me2, n, coup_cast<float>(c));
+  template <class T>
+  static constexpr int me_thr() { return stage_threads<P, T>(P::me_threads); }
+  template <class T>
+  static constexpr int int_thr() { return stage_threads<P, T>(kIntThreads); }
+
+  template <class K>
+  static cudaError_t allow_smem(K kernel, size_t bytes) {
+    if (bytes <= 48 * 1024) return cudaSuccess;
+    return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+  }
+  template <class T>
+  static cudaError_t me_t(int64_t n, const void* d_p, void* d_me2, const Coup<T>& c, cudaStream_t s) {
+    constexpr int TH = me_thr<T>();
+    constexpr size_t smem = stage_bytes<P, T, TH>();
+    cudaError_t err = allow_smem(me_kernel<P, T, TH>, smem);
+    if (err != cudaSuccess) return err;
+    const unsigned grid = (unsigned)((n + TH - 1) / TH);
+    me_kernel<P, T, TH><<<grid, TH, smem, s>>>((const T*)d_p, (T*)d_me2, n, c);
     return cudaGetLastError();
+  }
+  static cudaError_t me(int prec, int64_t n, const void* d_p, void* d_me2, const Coup<double>& c, cudaStream_t s) {
+    if (prec == HG_F64) return me_t<double>(n, d_p, d_me2, c, s);
+    return me_t<float>(n, d_p, d_me2, coup_cast<float>(c), s);
   }
   static cudaError_t ps(int prec, int64_t n, const PsConst& k, uint64_t seed, uint64_t first, void* d_p,
                         void* d_wps, uint8_t* d_pass, cudaStream_t s) {
     const unsigned grid = (unsigned)((n + 127) / 128);
     if (prec == HG_F64)
-      ps_kernel<P, double><<<grid, 128, 0, s>>>(k, seed, first, n, (double*)d_p, (double*)d_wps, d_pass);
+      ps_kernel<P, double, double><<<grid, 128, 0, s>>>(k, seed, first, n, (double*)d_p, (double*)d_wps, d_pass);
     else
-      ps_kernel<P, float><<<grid, 128, 0, s>>>(k, seed, first, n, (float*)d_p, (float*)d_wps, d_pass);
+      ps_kernel<P, float, float><<<grid, 128, 0, s>>>(k, seed, first, n, (float*)d_p, (float*)d_wps, d_pass);
     return cudaGetLastError();
+  }
+  template <class T>
+  static cudaError_t integrate_t(int64_t n, const PsConst& k, uint64_t seed, uint64_t first, const Coup<T>& c,
+                                 double wscale, double* d_partials, int nblocks, void* d_scratch, int64_t chunk,
+                                 cudaStream_t s) {
+    constexpr int TH = int_thr<T>();
+    constexpr size_t smem = stage_bytes<P, T, TH>();
+    if constexpr (P::n_stage == 0) {
+      integrate_kernel<P, T, TH><<<nblocks, TH, smem, s>>>(k, seed, first, n, c, wscale, d_partials);
+      return cudaGetLastError();
+    } else {
+      cudaError_t err = allow_smem(me_acc_kernel<P, T, TH>, smem);
+      if (err != cudaSuccess) return err;
+      for (int64_t off = 0; off < n; off += chunk) {
+        const int64_t m = n - off < chunk ? n - off : chunk;
+        T* d_p = (T*)d_scratch;                                      // [n_ext][4][m]
+        double* d_w = (double*)((char*)d_scratch + scratch_p_bytes<T>(chunk));
+        uint8_t* d_ok = (uint8_t*)(d_w + chunk);
+        ps_kernel<P, T, double><<<(unsigned)((m + 127) / 128), 128, 0, s>>>(k, seed, first + (uint64_t)off, m, d_p,
+                                                                            d_w, d_ok);
+        me_acc_kernel<P, T, TH><<<nblocks, TH, smem, s>>>(d_p, d_w, d_ok, m, c, wscale, off > 0 ? 1 : 0,
+                                                          d_partials);
+      }
+      return cudaGetLastError();
+    }
+  }
+  template <class T>
+  static constexpr size_t scratch_p_bytes(int64_t chunk) {
+    return ((size_t)chunk * P::n_ext * 4 * sizeof(T) + 255) / 256 * 256;
+  }
+  static size_t scratch_bytes_per_event(int prec) {
+    if (P::n_stage == 0) return 0;
+    return (size_t)P::n_ext * 4 * (prec == HG_F64 ? 8 : 4) + 8 + 1;
   }
   static cudaError_t integrate(int prec, int64_t n, const PsConst& k, uint64_t seed, uint64_t first,
                                const Coup<double>& c, double wscale, double* d_partials, int nblocks,
-                               cudaStream_t s) {
+                               void* d_scratch, int64_t chunk, cudaStream_t s) {
     if (prec == HG_F64)
-      integrate_kernel<P, double><<<nblocks, kIntThreads, 0, s>>>(k, seed, first, n, c, wscale, d_partials);
-    else
-      integrate_kernel<P, float><<<nblocks, kIntThreads, 0, s>>>(k, seed, first, n, coup_cast<float>(c), wscale,
-                                                                d_partials);
-    return cudaGetLastError();
+      return integrate_t<double>(n, k, seed, first, c, wscale, d_partials, nblocks, d_scratch, chunk, s);
+    return integrate_t<float>(n, k, seed, first, coup_cast<float>(c), wscale, d_partials, nblocks, d_scratch, chunk,
+                              s);
+  }
+  template <class T>
+  static cudaError_t int_blocks_t(int* out) {
+    constexpr int TH = int_thr<T>();
+    constexpr size_t smem = stage_bytes<P, T, TH>();
+    if constexpr (P::n_stage == 0) {
+      return cudaOccupancyMaxActiveBlocksPerMultiprocessor(out, integrate_kernel<P, T, TH>, TH, smem);
+    } else {
+      cudaError_t err = allow_smem(me_acc_kernel<P, T, TH>, smem);
+      if (err != cudaSuccess) return err;
+      return cudaOccupancyMaxActiveBlocksPerMultiprocessor(out, me_acc_kernel<P, T, TH>, TH, smem);
+    }
   }
   static cudaError_t int_blocks_per_sm(int prec, int* out) {
-    if (prec == HG_F64)
-      return cudaOccupancyMaxActiveBlocksPerMultiprocessor(out, integrate_kernel<P, double>, kIntThreads, 0);
-    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(out, integrate_kernel<P, float>, kIntThreads, 0);
+    return prec == HG_F64 ? int_blocks_t<double>(out) : int_blocks_t<float>(out);
   }
 };
 
@@ -142,7 +271,8 @@ template <class P>
 constexpr ProcVTable make_vtable(double flops_me, double flops_ps) {
   return ProcVTable{hg_process_info_t{P::n_ext, P::n_final, P::n_hel_total, P::n_hel_nonzero, P::n_diagrams,
                                       P::n_amplitudes, P::n_flows, P::n_draws, P::avg_factor, flops_me, flops_ps},
-                    &Launch<P>::me, &Launch<P>::ps, &Launch<P>::integrate, &Launch<P>::int_blocks_per_sm};
+                    &Launch<P>::me, &Launch<P>::ps, &Launch<P>::integrate, &Launch<P>::int_blocks_per_sm,
+                    &Launch<P>::scratch_bytes_per_event};
 }
 
 }  // namespace hg

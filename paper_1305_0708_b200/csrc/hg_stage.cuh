@@ -1,0 +1,135 @@
+// hg_stage.cuh -- per-event staging area for values that live across a helicity loop.
+//
+// The generated matrix element of a large process (W + 3 jets: 63 sub-currents, 54 amplitudes) has more values
+// alive across its helicity loops than fit in 255 registers; left to ptxas they become 3-5 KB of spill slots per
+// thread, which at 256 threads per SM is far larger than L1 (profiles/r01_notes.md: 105 GB of DRAM traffic per
+// launch from spills alone).  The generator therefore places every value that is produced outside a loop and
+// consumed inside it in a slot of this area and reloads it at each use, so that inside a loop body only the
+// operands of the current call are in registers.
+//
+// Device: the area is shared memory, laid out [slot][thread] so that a warp reads 32 consecutive words (no bank
+// conflicts).  Loads are volatile: the compiler may neither merge them nor hoist them out of the loops, which would
+// recreate the long live ranges.  Host (gen/flopcount, tests): a plain array per event.
+#pragma once
+#include "hg_cx.cuh"
+
+namespace hg {
+
+// no staging (small processes): every access is a compile error, the generator emits none
+struct NoStage {};
+
+#if defined(__CUDACC__)
+template <class T, int STRIDE>
+struct SmemStage {
+  T* b;  // shared memory + threadIdx.x
+  __device__ __forceinline__ T get(int s) const { return ((volatile T*)b)[s * STRIDE]; }
+  __device__ __forceinline__ void put(int s, T v) const { b[s * STRIDE] = v; }
+  // Block-wide rendezvous, emitted by the generator every few calls.  Nothing is exchanged: it keeps the warps of
+  // a block within a few hundred instructions of each other, so that they share instruction-cache lines (the
+  // generated code is 5-10x larger than the 32 KB L1.5 instruction cache; without it every warp streams its own
+  // copy of the code from L2, profiles/r01_notes.md section 3).  Every thread of the block must call me2().
+  __device__ __forceinline__ void sync() const { __syncthreads(); }
+};
+#endif
+template <class T>
+struct HostStage {
+  T* b;
+  T get(int s) const { return b[s]; }
+  void put(int s, T v) const { b[s] = v; }
+  void sync() const {}
+};
+
+template <class T, class St>
+HG_HD T ld_T(const St& st, int s) {
+  return st.get(s);
+}
+template <class T, class St>
+HG_HD void st_T(const St& st, int s, T v) {
+  st.put(s, v);
+}
+template <class T, class St>
+HG_HD cx<T> ld_cx(const St& st, int s) {
+  return mk<T>(st.get(s), st.get(s + 1));
+}
+template <class T, class St>
+HG_HD void st_cx(const St& st, int s, cx<T> v) {
+  st.put(s, v.re);
+  st.put(s + 1, v.im);
+}
+template <class T, class St>
+HG_HD Mom<T> ld_mom(const St& st, int s) {
+  return mkmom<T>(st.get(s), st.get(s + 1), st.get(s + 2), st.get(s + 3));
+}
+template <class T, class St>
+HG_HD void st_mom(const St& st, int s, const Mom<T>& v) {
+  st.put(s, v.e);
+  st.put(s + 1, v.x);
+  st.put(s + 2, v.y);
+  st.put(s + 3, v.z);
+}
+template <class T, class St>
+HG_HD Vc<T> ld_vec(const St& st, int s) {
+  Vc<T> v;
+  for (int i = 0; i < 4; ++i) v.c[i] = ld_cx<T>(st, s + 2 * i);
+  return v;
+}
+template <class T, class St>
+HG_HD void st_vec(const St& st, int s, const Vc<T>& v) {
+  for (int i = 0; i < 4; ++i) st_cx<T>(st, s + 2 * i, v.c[i]);
+}
+// spinor with slot mask M: only the non-zero slot pair(s) are kept
+template <int M, class T, class St>
+HG_HD Sp<T> ld_sp(const St& st, int s) {
+  Sp<T> f;
+  for (int i = 0; i < 4; ++i) f.c[i] = czero<T>();
+  int o = s;
+  if (M & SLOT_A) {
+    f.c[0] = ld_cx<T>(st, o);
+    f.c[1] = ld_cx<T>(st, o + 2);
+    o += 4;
+  }
+  if (M & SLOT_B) {
+    f.c[2] = ld_cx<T>(st, o);
+    f.c[3] = ld_cx<T>(st, o + 2);
+  }
+  return f;
+}
+template <int M, class T, class St>
+HG_HD void st_sp(const St& st, int s, const Sp<T>& f) {
+  int o = s;
+  if (M & SLOT_A) {
+    st_cx<T>(st, o, f.c[0]);
+    st_cx<T>(st, o + 2, f.c[1]);
+    o += 4;
+  }
+  if (M & SLOT_B) {
+    st_cx<T>(st, o, f.c[2]);
+    st_cx<T>(st, o + 2, f.c[3]);
+  }
+}
+// polarisation vector of a massless vector leg, helicity +1: eps^0 = 0 and eps^3 is real, so 5 words.
+// flip != 0 returns the helicity -1 vector -conj(eps) (vflip).
+template <class T, class St>
+HG_HD void st_pol(const St& st, int s, const Vc<T>& e) {
+  st.put(s, e.c[1].re);
+  st.put(s + 1, e.c[1].im);
+  st.put(s + 2, e.c[2].re);
+  st.put(s + 3, e.c[2].im);
+  st.put(s + 4, e.c[3].re);
+}
+template <class T, class St>
+HG_HD Vc<T> ld_pol(const St& st, int s, int flip) {
+  Vc<T> v;
+  v.c[0] = czero<T>();
+  v.c[1] = mk<T>(st.get(s), st.get(s + 1));
+  v.c[2] = mk<T>(st.get(s + 2), st.get(s + 3));
+  v.c[3] = mk<T>(st.get(s + 4), T(0));
+  if (flip) {
+    v.c[1].re = -v.c[1].re;
+    v.c[2].re = -v.c[2].re;
+    v.c[3].re = -v.c[3].re;
+  }
+  return v;
+}
+
+}  // namespace hg

@@ -175,30 +175,152 @@ def _popcount(m):
 
 
 class CodeGen(Emitter):
-    """Emits `template <class T> HG_HD T me2_<name>(const Mom<T>* p, const Coup<T>& c)`."""
+    """Emits `template <class T, class St> HG_HD T me2_<name>(const Mom<T>* p, const Coup<T>& c, const St& st)`.
 
+    stage=True: every value produced outside a helicity loop and consumed inside one is kept in the staging area
+    `st` (csrc/hg_stage.cuh; shared memory on the device) and reloaded at each use; stage=False: plain SSA values,
+    liveness left to nvcc (small processes)."""
+
+    SIZES = {'T': 1, 'cx<T>': 2, 'Mom<T>': 4, 'Vc<T>': 8, 'pol': 5}
+    SYNC_EVERY = 4     # staged mode: block rendezvous after this many calls (instruction-cache sharing)
+
+    def __init__(self, diag, stage=False, kfromp=False):
+        super().__init__(diag)
+        self.stage = stage
+        self.kfromp = stage and kfromp   # inside loops rebuild internal momenta from staged external momenta
+
+    # ------------------------------------------------------------------ value registry / operand access
+    def _reg(self, name, ctype, depth, mask=AB, region=None, pol_of=None, hvar=None):
+        if name not in self.vals:
+            self.vals[name] = dict(name=name, ctype=ctype, depth=depth, mask=mask, slot=None,
+                                   region=(0 if depth == 0 else 1) if region is None else region,
+                                   pol_of=pol_of, hvar=hvar)
+        return self.vals[name]
+
+    def _size(self, v):
+        if v['ctype'] == 'Sp<T>':
+            return 8 if v['mask'] == AB else 4
+        return self.SIZES[v['ctype']]
+
+    def _slot(self, v):
+        """Slot expression of a staged value (allocated on first use)."""
+        if v['slot'] is None:
+            r = v['region']
+            v['slot'] = self.n_slots[r]
+            self.n_slots[r] += self._size(v)
+            self.max_slots[r] = max(self.max_slots[r], self.n_slots[r])
+        return str(v['slot']) if v['region'] == 0 else 'L + %d' % v['slot']
+
+    def _load_expr(self, v):
+        ct = v['ctype']
+        if ct == 'Sp<T>':
+            return 'ld_sp<%d, T>(st, %s)' % (v['mask'], self._slot(v))
+        fn = {'T': 'ld_T', 'cx<T>': 'ld_cx', 'Mom<T>': 'ld_mom', 'Vc<T>': 'ld_vec'}[ct]
+        return '%s<T>(st, %s)' % (fn, self._slot(v))
+
+    def _store_line(self, v):
+        ct = v['ctype']
+        if ct == 'pol':
+            return 'st_pol<T>(st, %s, %s);' % (self._slot(v), v['name'])
+        if ct == 'Sp<T>':
+            return 'st_sp<%d, T>(st, %s, %s);' % (v['mask'], self._slot(v), v['name'])
+        fn = {'T': 'st_T', 'cx<T>': 'st_cx', 'Mom<T>': 'st_mom', 'Vc<T>': 'st_vec'}[ct]
+        return '%s<T>(st, %s, %s);' % (fn, self._slot(v), v['name'])
+
+    def _ref(self, name):
+        """Text by which the op being emitted (at loop depth self.cur_depth) reads value `name`."""
+        v = self.vals[name]
+        if not self.stage or v['depth'] >= self.cur_depth:
+            return name
+        alias = 'a%d' % len(self.cur_loads)
+        if v['pol_of'] is not None:      # helicity state of a looped massless vector leg: from its eps(+1)
+            e = self.vals[v['pol_of']]
+            self.cur_loads.append('const Vc<T> %s = ld_pol<T>(st, %s, %s);' % (alias, self._slot(e), v['hvar']))
+        elif v['ctype'] == 'pol':
+            self.cur_loads.append('const Vc<T> %s = ld_pol<T>(st, %s, 0);' % (alias, self._slot(v)))
+        else:
+            self.cur_loads.append('const %s %s = %s;' % (v['ctype'], alias, self._load_expr(v)))
+        return alias
+
+    def _begin(self, depth):
+        self.cur_depth = depth
+        self.cur_loads = []
+
+    # ------------------------------------------------------------------ driver
     def generate(self):
+        self.vals = {}
+        self.n_slots = [0, 0]
+        self.max_slots = [0, 0]
         self.need_K = set()       # masks whose summed momentum is needed
-        self.need_Kn = set()      # masks whose negated momentum is needed (row spinor propagators)
+        self.need_P = set()       # external legs whose momentum is read inside loops (kfromp)
         self.need_d = {}          # (mask, field) -> variable name of the propagator factor
         self.need_rm2 = set()     # mass names whose 1/m^2 is needed
-        self.body = []
         self.shared = {}          # key -> name of depth-0 values already emitted
-        self.shared_lines = []
+        self.shared_items = []
         dyn = self.dynamic
         self.depth_of_leg = {l: i + 1 for i, l in enumerate(dyn)}
+        for l in dyn:
+            lg = self.legs[l]
+            if lg.particle.spin == 'V' and not lg.particle.mass:
+                self._reg('e%d' % l, 'pol', 0)
+                if self.stage:
+                    self._slot(self.vals['e%d' % l])
+                self._reg('x%d' % l, 'Vc<T>', self.depth_of_leg[l], pol_of='e%d' % l, hvar='h%d' % l)
+            elif self.stage:
+                raise NotImplementedError('staged mode: looped legs must be massless vector bosons')
+            else:
+                self._reg('x%d' % l, {'V': 'Vc<T>', 'F': 'Sp<T>', 'S': 'cx<T>'}[lg.particle.spin],
+                          self.depth_of_leg[l])
         flows, cmat, cden = self.colour_matrix()
         self.flows = flows
-        body = self.body
+        variants = []
         for vi, (hel, roots) in enumerate(self.variants):
-            self._emit_variant(vi, hel, roots, cmat)
+            self.n_slots[1] = 0       # loop-level slots are reused by every static-helicity variant
+            variants.append(self._emit_variant(vi, hel, roots, cmat))
+        pre = self._preamble()
         out = []
-        out += self._preamble()
-        out += self.shared_lines
+        if self.stage:
+            out.append('  constexpr int L = %d;  // first slot of the loop-level values' % self.max_slots[0])
+        out += self._render_items(pre, '  ')
+        out += self._render_items(self.shared_items, '  ')
         out.append('  T me = T(0);')
-        out += body
+        for var in variants:
+            out += self._render_variant(var)
         scale = self.avg_factor() / cden
         out.append('  return me * T(%s);' % _lit(scale))
+        self.n_stage = self.max_slots[0] + self.max_slots[1] if self.stage else 0
+        return out
+
+    def _render_items(self, items, ind):
+        """items: ('raw', text) | ('def', name, expr, loads) | ('blk', [lines], loads)."""
+        out = []
+        nsince = 0
+        for it in items:
+            if self.stage and it[0] != 'raw':
+                nsince += 1
+                if nsince > self.SYNC_EVERY:
+                    out.append(ind + 'st.sync();')
+                    nsince = 1
+            if it[0] == 'raw':
+                out.append(ind + it[1])
+            elif it[0] == 'def':
+                _, name, expr, loads = it
+                v = self.vals[name]
+                ct = 'Vc<T>' if v['ctype'] == 'pol' else v['ctype']
+                if loads:
+                    out.append(ind + '%s %s;' % (ct, name))
+                    out.append(ind + '{ ' + ' '.join(loads))
+                    out.append(ind + '  %s = %s; }' % (name, expr))
+                else:
+                    out.append(ind + 'const %s %s = %s;' % (ct, name, expr))
+                if self.stage and v['slot'] is not None:
+                    out.append(ind + self._store_line(v))
+            else:
+                _, lines, loads = it
+                out.append(ind + '{ ' + ' '.join(loads))
+                for ln in lines:
+                    out.append(ind + '  ' + ln)
+                out.append(ind + '}')
         return out
 
     # ------------------------------------------------------------------ helpers
@@ -211,21 +333,37 @@ class CodeGen(Emitter):
     def _helcode(self, mask, hel):
         return ''.join('p' if hel[l] > 0 else 'm' for l in bits(mask) if l in hel)
 
-    def _K(self, mask):
+    def _K(self, mask, neg=False):
+        if self.kfromp and self.cur_depth > 0:
+            # sum of at most n/2 external momenta (momentum conservation: K(mask) = -K(complement))
+            n = self.dg.n
+            use, sg = (mask, 1) if _popcount(mask) <= n - _popcount(mask) else (self.dg.full & ~mask, -1)
+            if neg:
+                sg = -sg
+            terms = []
+            for l in bits(use):
+                self.need_P.add(l)
+                self._reg('P%d' % l, 'Mom<T>', 0)
+                s_l = sg * (1 if self.legs[l].state == 'in' else -1)
+                terms.append(('+' if s_l > 0 else '-', self._ref('P%d' % l)))
+            txt = ('-' if terms[0][0] == '-' else '') + terms[0][1]
+            for sign, t in terms[1:]:
+                txt += ' %s %s' % (sign, t)
+            return '(%s)' % txt if len(terms) > 1 or terms[0][0] == '-' else txt
         self.need_K.add(mask)
-        return 'K%d' % mask
+        self._reg('K%d' % mask, 'Mom<T>', 0)
+        return ('-' if neg else '') + self._ref('K%d' % mask)
 
     def _Kn(self, mask):
-        self.need_K.add(mask)
-        self.need_Kn.add(mask)
-        return 'Kn%d' % mask
+        return self._K(mask, neg=True)
 
     def _d(self, nd):
         p = nd.particle
         key = (nd.mask, p.mass, p.width, p.spin)
         if key not in self.need_d:
             self.need_d[key] = 'd%d_%s%s' % (nd.mask, p.spin.lower(), p.mass or '0')
-        return self.need_d[key]
+            self._reg(self.need_d[key], 'cx<T>' if p.width else 'T', 0)
+        return self._ref(self.need_d[key])
 
     def _mass(self, p):
         return 'c.%s' % p.mass if p.mass else 'T(0)'
@@ -234,7 +372,8 @@ class CodeGen(Emitter):
         if not p.mass:
             return 'T(0)'
         self.need_rm2.add(p.mass)
-        return 'rm2_%s' % p.mass
+        self._reg('rm2_%s' % p.mass, 'T', 0)
+        return self._ref('rm2_%s' % p.mass)
 
     @staticmethod
     def _cpl(name):
@@ -262,7 +401,7 @@ class CodeGen(Emitter):
     def _node_expr(self, nd, vi, hel):
         v = nd.vertex
         by_slot = dict(zip(nd.slots, nd.children))
-        nm = lambda ch: self._name(ch, vi, hel)
+        nm = lambda ch: self._ref(self._name(ch, vi, hel))
         mk = lambda ch: self._node_mask(ch, hel, self.memo)
         p = nd.particle
         massive = 'true' if p.mass else 'false'
@@ -278,8 +417,11 @@ class CodeGen(Emitter):
                 return 'fvoxxx<%d, %d, %s>(%s, %s, %s, %s, %s, %s, %s)' % (
                     mk(row), g, massive, nm(row), nm(vec), gl, gr, self._Kn(nd.mask), self._mass(p), self._d(nd))
             row, col = by_slot[0], by_slot[1]
-            return 'jioxxx<%d, %d, %d, %s>(%s, %s, %s, %s, %s, %s, %s)' % (
-                mk(col), mk(row), g, massive, nm(col), nm(row), gl, gr, self._K(nd.mask), self._rm2(p), self._d(nd))
+            if p.mass:
+                return 'jioxxx<%d, %d, %d, true>(%s, %s, %s, %s, %s, %s, %s)' % (
+                    mk(col), mk(row), g, nm(col), nm(row), gl, gr, self._K(nd.mask), self._rm2(p), self._d(nd))
+            return 'jioxx0<%d, %d, %d>(%s, %s, %s, %s, %s)' % (
+                mk(col), mk(row), g, nm(col), nm(row), gl, gr, self._d(nd))
         if v.kind == 'VVV':
             a, b = by_slot[(nd.out_slot + 1) % 3], by_slot[(nd.out_slot + 2) % 3]
             return 'jvvxxx<%s>(%s, %s, %s, %s, %s, %s, %s)' % (
@@ -297,7 +439,7 @@ class CodeGen(Emitter):
     def _root_expr(self, rt, vi, hel):
         v = rt.vertex
         by_slot = dict(zip(rt.slots, rt.children))
-        nm = lambda ch: self._name(ch, vi, hel)
+        nm = lambda ch: self._ref(self._name(ch, vi, hel))
         mk = lambda ch: self._node_mask(ch, hel, self.memo)
         if v.kind == 'FFV':
             row, col, vec = by_slot[0], by_slot[1], by_slot[2]
@@ -327,7 +469,7 @@ class CodeGen(Emitter):
     def _root_current_expr(self, rt, vi, hel):
         v = rt.vertex
         by_slot = dict(zip(rt.slots, rt.children))
-        nm = lambda ch: self._name(ch, vi, hel)
+        nm = lambda ch: self._ref(self._name(ch, vi, hel))
         mk = lambda ch: self._node_mask(ch, hel, self.memo)
         last = self.dg.last
         is_last = lambda ch: ch.is_leaf and ch.leg == last
@@ -364,7 +506,7 @@ class CodeGen(Emitter):
         dyn = self.dynamic
         cbc = self.closes_by_current()
         k = len(dyn) - 1 if cbc else len(dyn)   # number of helicity loops
-        levels = [[] for _ in range(k + 1)]     # lines per loop depth
+        levels = [[] for _ in range(k + 1)]     # items per loop depth
         done = set()
 
         def need(nd):
@@ -380,14 +522,16 @@ class CodeGen(Emitter):
                 return
             for ch in nd.children:
                 need(ch)
+            self._reg(name, self._wtype_decl(nd), dep, mask=self._node_mask(nd, hel, self.memo))
+            self._begin(dep)
             expr = self._leaf_expr(nd, hel) if nd.is_leaf else self._node_expr(nd, vi, hel)
-            line = 'const %s %s = %s;' % (self._wtype_decl(nd), name, expr)
+            item = ('def', name, expr, self.cur_loads)
             if dep == 0:
                 self.shared[name] = True
-                self.shared_lines.append('  ' + line)
+                self.shared_items.append(item)
             else:
                 done.add(nd.uid)
-                levels[dep].append(line)
+                levels[dep].append(item)
 
         nf = len(self.flows)
         fidx = {w: i for i, w in enumerate(self.flows)}
@@ -396,30 +540,31 @@ class CodeGen(Emitter):
         for rt in roots:
             for ch in rt.children:
                 need(ch)
+            self._begin(k)
+            lines = []
             if cbc:
-                inner.append('{ const Vc<T> b = %s;' % self._root_current_expr(rt, vi, hel))
-                inner.append('  cx<T> rb, ib;')
-                inner.append('  close_proj(e%d, b, rb, ib);' % last)
+                lines.append('const Vc<T> b = %s;' % self._root_current_expr(rt, vi, hel))
+                lines.append('cx<T> rb, ib;')
+                lines.append('close_proj(%s, b, rb, ib);' % self._ref('e%d' % last))
                 for w, cf in sorted(rt.colour.terms.items()):
                     f = fidx[w]
                     if cf == 1:
-                        inner.append('  X%d = X%d + rb; Y%d = Y%d + ib;' % (f, f, f, f))
+                        lines.append('X%d = X%d + rb; Y%d = Y%d + ib;' % (f, f, f, f))
                     elif cf == -1:
-                        inner.append('  X%d = X%d - rb; Y%d = Y%d - ib;' % (f, f, f, f))
+                        lines.append('X%d = X%d - rb; Y%d = Y%d - ib;' % (f, f, f, f))
                     else:
-                        inner.append('  X%d = X%d + T(%d) * rb; Y%d = Y%d + T(%d) * ib;' % (f, f, cf, f, f, cf))
-                inner.append('}')
-                continue
-            inner.append('{ const cx<T> a = %s;' % self._root_expr(rt, vi, hel))
-            for w, cf in sorted(rt.colour.terms.items()):
-                f = fidx[w]
-                if cf == 1:
-                    inner.append('  j%d = j%d + a;' % (f, f))
-                elif cf == -1:
-                    inner.append('  j%d = j%d - a;' % (f, f))
-                else:
-                    inner.append('  j%d = j%d + T(%d) * a;' % (f, f, cf))
-            inner.append('}')
+                        lines.append('X%d = X%d + T(%d) * rb; Y%d = Y%d + T(%d) * ib;' % (f, f, cf, f, f, cf))
+            else:
+                lines.append('const cx<T> a = %s;' % self._root_expr(rt, vi, hel))
+                for w, cf in sorted(rt.colour.terms.items()):
+                    f = fidx[w]
+                    if cf == 1:
+                        lines.append('j%d = j%d + a;' % (f, f))
+                    elif cf == -1:
+                        lines.append('j%d = j%d - a;' % (f, f))
+                    else:
+                        lines.append('j%d = j%d + T(%d) * a;' % (f, f, cf))
+            inner.append(('blk', lines, self.cur_loads))
         # colour contraction (symmetric form)
         tail = []
         if cbc:
@@ -443,16 +588,19 @@ class CodeGen(Emitter):
             accdecl = 'cx<T> ' + ', '.join('X%d = czero<T>(), Y%d = czero<T>()' % (f, f) for f in range(nf)) + ';'
         else:
             accdecl = 'cx<T> ' + ', '.join('j%d = czero<T>()' % f for f in range(nf)) + ';'
-        # assemble
-        b = self.body
+        return dict(hel=hel, levels=levels, tail=tail, k=k, accdecl=accdecl)
+
+    def _render_variant(self, var):
+        dyn = self.dynamic
+        k, levels = var['k'], var['levels']
+        b = []
         ind = '  '
         b.append(ind + '{  // static helicities: ' +
-                 ', '.join('%s(%d)=%+d' % (self.legs[l].name, l, h) for l, h in sorted(hel.items())))
+                 ', '.join('%s(%d)=%+d' % (self.legs[l].name, l, h) for l, h in sorted(var['hel'].items())))
         ind += '  '
         if k == 0:
-            b.append(ind + accdecl)
-        for line in levels[0]:
-            b.append(ind + line)
+            b.append(ind + var['accdecl'])
+        b += self._render_items(levels[0], ind)
         for d in range(1, k + 1):
             leg = dyn[d - 1]
             lg = self.legs[leg]
@@ -460,23 +608,27 @@ class CodeGen(Emitter):
             b.append(ind + '#pragma unroll 1')
             b.append(ind + 'for (int h%d = 0; h%d < %d; ++h%d) {' % (leg, leg, nh, leg))
             ind += '  '
+            if self.stage:
+                b.append(ind + 'st.sync();')
             b.append(ind + self._dyn_leaf_decl(lg))
             if d == k:
-                b.append(ind + accdecl)
-            for line in levels[d]:
-                b.append(ind + line)
-        for line in tail:
+                b.append(ind + var['accdecl'])
+            b += self._render_items(levels[d], ind)
+        for line in var['tail']:
             b.append(ind + line)
         for d in range(k):
             ind = ind[:-2]
             b.append(ind + '}')
         ind = ind[:-2]
         b.append(ind + '}')
+        return b
 
     def _dyn_leaf_decl(self, lg):
         p = lg.particle
         i = lg.index
         if p.spin == 'V' and not p.mass:
+            if self.stage:
+                return 'const Vc<T> x%d = ld_pol<T>(st, %s, h%d);' % (i, self._slot(self.vals['e%d' % i]), i)
             return 'const Vc<T> x%d = h%d ? vflip(e%d) : e%d;' % (i, i, i, i)
         if p.spin == 'V':
             nsv = -1 if lg.state == 'in' else 1
@@ -488,15 +640,23 @@ class CodeGen(Emitter):
 
     # ------------------------------------------------------------------ per-event, helicity independent part
     def _preamble(self):
+        """Items of loop depth 0: momenta of internal lines, invariants, propagator factors, eps(+1) of looped legs."""
+        self._begin(0)
         L = []
+        raw = lambda t: L.append(('raw', t))
+
+        def define(name, ctype, expr):
+            self._reg(name, ctype, 0)
+            L.append(('def', name, expr, []))
+
         n = self.dg.n
         sgn = {l.index: (1 if l.state == 'in' else -1) for l in self.legs}
+        for l in sorted(self.need_P):
+            define('P%d' % l, 'Mom<T>', 'p[%d]' % l)
         # momenta of sub-sets (all-incoming: initial +p, final -p)
         have = {}
         for m in sorted(self.need_K, key=lambda m: (_popcount(m), m)):
-            self._emit_K(m, have, L, sgn)
-        for m in sorted(self.need_Kn):
-            L.append('  const Mom<T> Kn%d = -K%d;' % (m, m))
+            self._emit_K(m, have, define, sgn)
         # invariants
         pairs = set()
         q2 = {}
@@ -510,46 +670,46 @@ class CodeGen(Emitter):
                         pairs.add((ls[a], ls[b2]))
         units = sorted({l for pr in pairs for l in pr if not self.legs[l].particle.mass})
         for l in units:
-            L.append('  const Mom<T> n%d = unit0(p[%d]);' % (l, l))
+            raw('const Mom<T> n%d = unit0(p[%d]);' % (l, l))
         for (a, b2) in sorted(pairs):
             s = '' if sgn[a] * sgn[b2] > 0 else '-'
             if not self.legs[a].particle.mass and not self.legs[b2].particle.mass:
-                L.append('  const T t%d_%d = %stwo_dot0(n%d, n%d);' % (a, b2, s, a, b2))
+                raw('const T t%d_%d = %stwo_dot0(n%d, n%d);' % (a, b2, s, a, b2))
             else:
-                L.append('  const T t%d_%d = %sT(2) * mdot(p[%d], p[%d]);' % (a, b2, s, a, b2))
+                raw('const T t%d_%d = %sT(2) * mdot(p[%d], p[%d]);' % (a, b2, s, a, b2))
         for m, use in sorted(q2.items()):
             ls = list(bits(use))
             terms = ['t%d_%d' % (ls[a], ls[b2]) for a in range(len(ls)) for b2 in range(a + 1, len(ls))]
             for l in ls:
                 if self.legs[l].particle.mass:
                     terms.append('c.%s * c.%s' % (self.legs[l].particle.mass, self.legs[l].particle.mass))
-            L.append('  const T q2_%d = %s;' % (m, ' + '.join(terms)))
+            raw('const T q2_%d = %s;' % (m, ' + '.join(terms)))
         for mass in sorted(self.need_rm2):
-            L.append('  const T rm2_%s = hrcp(c.%s * c.%s);' % (mass, mass, mass))
+            define('rm2_%s' % mass, 'T', 'hrcp(c.%s * c.%s)' % (mass, mass))
         for (m, mass, width, spin), name in sorted(self.need_d.items()):
             sign = '' if spin == 'V' else '-'
             den = 'q2_%d' % m if not mass else '(q2_%d - c.%s * c.%s)' % (m, mass, mass)
             if width:
-                L.append('  const cx<T> %s = %scrcp(%s, c.%s * c.%s);' % (name, sign, den, mass, width))
+                define(name, 'cx<T>', '%scrcp(%s, c.%s * c.%s)' % (sign, den, mass, width))
             else:
-                L.append('  const T %s = %shrcp(%s);' % (name, sign, den))
+                define(name, 'T', '%shrcp(%s)' % (sign, den))
         # polarisation vectors of looped massless vector legs (helicity +1; -1 by vflip)
         for l in self.dynamic:
             lg = self.legs[l]
             if lg.particle.spin == 'V' and not lg.particle.mass:
-                L.append('  const Vc<T> e%d = vxxxxx<T>(p[%d], T(0), 1, %d);' % (l, l, -1 if lg.state == 'in' else 1))
+                define('e%d' % l, 'pol', 'vxxxxx<T>(p[%d], T(0), 1, %d)' % (l, -1 if lg.state == 'in' else 1))
         return L
 
-    def _emit_K(self, m, have, L, sgn):
+    def _emit_K(self, m, have, define, sgn):
         if m in have:
             return
         hi = max(bits(m))
         rest = m & ~(1 << hi)
         if rest == 0:
-            L.append('  const Mom<T> K%d = %sp[%d];' % (m, '' if sgn[hi] > 0 else '-', hi))
+            define('K%d' % m, 'Mom<T>', '%sp[%d]' % ('' if sgn[hi] > 0 else '-', hi))
         else:
-            self._emit_K(rest, have, L, sgn)
-            L.append('  const Mom<T> K%d = K%d %s p[%d];' % (m, rest, '+' if sgn[hi] > 0 else '-', hi))
+            self._emit_K(rest, have, define, sgn)
+            define('K%d' % m, 'Mom<T>', 'K%d %s p[%d]' % (rest, '+' if sgn[hi] > 0 else '-', hi))
         have[m] = True
 
 

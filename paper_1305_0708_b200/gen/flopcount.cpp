@@ -32,14 +32,18 @@ void run(double rs) {
     P::gen(k, 20130507ull, (unsigned long long)e, p);
     Mom<Cnt> q[P::n_ext];
     for (int l = 0; l < P::n_ext; ++l) q[l] = mkmom<Cnt>(Cnt(p[l].e), Cnt(p[l].x), Cnt(p[l].y), Cnt(p[l].z));
+    static Cnt sc[P::n_stage + 1];
+    static double sd[P::n_stage + 1];
+    const HostStage<Cnt> stc{sc};
+    const HostStage<double> std_{sd};
     Cnt::n() = 0;
-    const Cnt r = P::template me2<Cnt>(q, cc);
+    const Cnt r = P::template me2<Cnt>(q, cc, stc);
     const long long f = Cnt::n();
     if (e == 0 || f < lo) lo = f;
     if (e == 0 || f > hi) hi = f;
     sum += f;
     v_c = r.v;
-    v_d = P::template me2<double>(p, cd);
+    v_d = P::template me2<double>(p, cd, std_);
   }
   printf("%d %lld %.1f %lld %.17g %.17g\n", P::pid, lo, (double)sum / N, hi, v_d, v_c);
 }
