@@ -16,29 +16,57 @@
 
 namespace hg {
 
-// Threads per block of a kernel that evaluates me2<T>.  A staged process needs P::n_stage words of shared memory
-// per thread, which is what limits the warps resident on an SM (227 KB).  All of them go into one block (two
-// blocks when more than 6 fit) because the warps of a block run the generated code in step (SmemStage::sync).
+// Threads per block of a kernel that evaluates me2<T>.
+//
+// A staged process (P::n_stage > 0) keeps P::n_stage words per EVENT in shared memory, which is what limits the
+// events in flight on an SM (227 KB).  Each event is evaluated by a PAIR of warps (pair split): warps 2g and 2g+1
+// of a block hold the same 32 events, share their staging area, and take one iteration each of the innermost
+// helicity loop (SmemStage::lo/hi), which is ~90 % of the work; the helicity-independent part is computed by both
+// (they write identical values to the same slots).  Two warps per scheduler are what hides the instruction-fetch
+// stall at every 128-byte line of the 170 KB straight-line code (profiles/r01_notes.md section 3).
 constexpr int kSmemPerSM = 227 * 1024;
+template <class P>
+constexpr int kSplit = P::n_stage > 0 ? 2 : 1;
 template <class P, class T>
 constexpr int stage_threads(int want) {
   if (P::n_stage == 0) return want;
-  const int fit = kSmemPerSM / (P::n_stage * (int)sizeof(T) * 32);
-  const int w = fit <= 6 ? fit : (fit <= 12 ? fit / 2 : 6);
-  return 32 * (w < 1 ? 1 : w);
+  const int groups = kSmemPerSM / (P::n_stage * (int)sizeof(T) * 32);  // 32-event groups that fit on an SM
+  const int g = groups < 1 ? 1 : (groups > 4 ? 4 : groups);
+  return 64 * g;
 }
 template <class P, class T, int THREADS>
 constexpr size_t stage_bytes() {
-  return (size_t)P::n_stage * sizeof(T) * THREADS;
+  return (size_t)P::n_stage * sizeof(T) * (THREADS / kSplit<P>);
+}
+// index of this thread's event within the block, and whether this thread owns the event's result
+template <class P>
+__device__ __forceinline__ int ev_local() {
+  if constexpr (P::n_stage > 0) return ((threadIdx.x >> 6) << 5) | (threadIdx.x & 31);
+  return threadIdx.x;
+}
+template <class P>
+__device__ __forceinline__ bool ev_owner() {
+  if constexpr (P::n_stage > 0) return ((threadIdx.x >> 5) & 1) == 0;
+  return true;
 }
 
-// me2 of one event with the staging area of this thread (shared memory laid out [slot][thread], hg_stage.cuh)
+// me2 of one event.  Staged: the staging area of the event is shared memory laid out [slot][event] (hg_stage.cuh);
+// every thread of the block must call; the total is returned to the owner thread of the pair.
 template <class P, class T, int THREADS>
 __device__ __forceinline__ T me2_event(const Mom<T>* q, const Coup<T>& c) {
   if constexpr (P::n_stage > 0) {
+    constexpr int EPB = THREADS / 2;
     extern __shared__ __align__(16) unsigned char hg_stage_smem[];
-    const SmemStage<T, THREADS> st{reinterpret_cast<T*>(hg_stage_smem) + threadIdx.x};
-    return P::template me2<T>(q, c, st);
+    __shared__ T comb[EPB];
+    const int ev = ev_local<P>();
+    const int half = (threadIdx.x >> 5) & 1;
+    const SmemStage<T, EPB> st{reinterpret_cast<T*>(hg_stage_smem) + ev, half};
+    T r = P::template me2<T>(q, c, st);
+    if (half) comb[ev] = r;
+    __syncthreads();
+    if (!half) r += comb[ev];
+    __syncthreads();  // comb and the staging area are free for the next event
+    return r;
   } else {
     return P::template me2<T>(q, c, NoStage{});
   }
@@ -47,14 +75,15 @@ __device__ __forceinline__ T me2_event(const Mom<T>* q, const Coup<T>& c) {
 template <class P, class T, int THREADS>
 __global__ void __launch_bounds__(THREADS) me_kernel(const T* __restrict__ p, T* __restrict__ me2, int64_t n,
                                                      const Coup<T> c) {
-  const int64_t e0 = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  constexpr int EPB = THREADS / kSplit<P>;
+  const int64_t e0 = (int64_t)blockIdx.x * EPB + ev_local<P>();
   const int64_t e = e0 < n ? e0 : n - 1;  // no early exit: a staged me2 holds block-wide rendezvous
   Mom<T> q[P::n_ext];
 #pragma unroll
   for (int l = 0; l < P::n_ext; ++l)
     q[l] = mkmom<T>(p[(l * 4 + 0) * n + e], p[(l * 4 + 1) * n + e], p[(l * 4 + 2) * n + e], p[(l * 4 + 3) * n + e]);
   const T r = me2_event<P, T, THREADS>(q, c);
-  if (e0 < n) me2[e0] = r;
+  if (e0 < n && ev_owner<P>()) me2[e0] = r;
 }
 
 template <class P, class T, class W>
@@ -143,8 +172,9 @@ __global__ void __launch_bounds__(THREADS) me_acc_kernel(const T* __restrict__ p
                                                          const Coup<T> c, double wscale, int add,
                                                          double* __restrict__ partials) {
   double sw = 0.0, sw2 = 0.0, np = 0.0;
-  for (int64_t base = (int64_t)blockIdx.x * THREADS; base < n; base += (int64_t)gridDim.x * THREADS) {
-    const int64_t e0 = base + threadIdx.x;
+  constexpr int EPB = THREADS / kSplit<P>;
+  for (int64_t base = (int64_t)blockIdx.x * EPB; base < n; base += (int64_t)gridDim.x * EPB) {
+    const int64_t e0 = base + ev_local<P>();
     const int64_t e = e0 < n ? e0 : n - 1;
     const bool ok = e0 < n && pass[e] != 0;
     if (__syncthreads_or(ok)) {
@@ -154,7 +184,7 @@ __global__ void __launch_bounds__(THREADS) me_acc_kernel(const T* __restrict__ p
         q[l] = mkmom<T>(p[(l * 4 + 0) * n + e], p[(l * 4 + 1) * n + e], p[(l * 4 + 2) * n + e],
                         p[(l * 4 + 3) * n + e]);
       const double w = (double)me2_event<P, T, THREADS>(q, c) * wps[e] * wscale;
-      if (ok) {
+      if (ok && ev_owner<P>()) {
         sw += w;
         sw2 += w * w;
         np += 1.0;
@@ -192,7 +222,8 @@ struct Launch {
     constexpr size_t smem = stage_bytes<P, T, TH>();
     cudaError_t err = allow_smem(me_kernel<P, T, TH>, smem);
     if (err != cudaSuccess) return err;
-    const unsigned grid = (unsigned)((n + TH - 1) / TH);
+    constexpr int EPB = TH / kSplit<P>;
+    const unsigned grid = (unsigned)((n + EPB - 1) / EPB);
     me_kernel<P, T, TH><<<grid, TH, smem, s>>>((const T*)d_p, (T*)d_me2, n, c);
     return cudaGetLastError();
   }

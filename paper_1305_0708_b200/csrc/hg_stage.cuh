@@ -21,7 +21,10 @@ struct NoStage {};
 #if defined(__CUDACC__)
 template <class T, int STRIDE>
 struct SmemStage {
-  T* b;  // shared memory + threadIdx.x
+  T* b;      // shared memory + index of the event in the block
+  int half;  // which half of the innermost helicity loop this warp evaluates (pair split, hg_process_impl.cuh)
+  __device__ __forceinline__ int lo() const { return half; }
+  __device__ __forceinline__ int hi() const { return half + 1; }
   __device__ __forceinline__ T get(int s) const { return ((volatile T*)b)[s * STRIDE]; }
   __device__ __forceinline__ void put(int s, T v) const { b[s * STRIDE] = v; }
   // Block-wide rendezvous, emitted by the generator every few calls.  Nothing is exchanged: it keeps the warps of
@@ -36,6 +39,8 @@ struct HostStage {
   T* b;
   T get(int s) const { return b[s]; }
   void put(int s, T v) const { b[s] = v; }
+  int lo() const { return 0; }
+  int hi() const { return 2; }
   void sync() const {}
 };
 

@@ -273,6 +273,11 @@ class CodeGen(Emitter):
                           self.depth_of_leg[l])
         flows, cmat, cden = self.colour_matrix()
         self.flows = flows
+        if self.stage:
+            # the kernels split the innermost loop over a pair of warps (csrc/hg_process_impl.cuh)
+            nloops = len(dyn) - 1 if self.closes_by_current() else len(dyn)
+            if nloops < 1 or len(self.nhel[dyn[nloops - 1]]) != 2:
+                raise NotImplementedError('staged mode needs an innermost helicity loop of two states')
         variants = []
         for vi, (hel, roots) in enumerate(self.variants):
             self.n_slots[1] = 0       # loop-level slots are reused by every static-helicity variant
@@ -606,7 +611,11 @@ class CodeGen(Emitter):
             lg = self.legs[leg]
             nh = len(self.nhel[leg])
             b.append(ind + '#pragma unroll 1')
-            b.append(ind + 'for (int h%d = 0; h%d < %d; ++h%d) {' % (leg, leg, nh, leg))
+            if self.stage and d == k and nh == 2:
+                # innermost loop: on the device its two iterations run in the two warps of a pair (st.lo/st.hi)
+                b.append(ind + 'for (int h%d = st.lo(); h%d < st.hi(); ++h%d) {' % (leg, leg, leg))
+            else:
+                b.append(ind + 'for (int h%d = 0; h%d < %d; ++h%d) {' % (leg, leg, nh, leg))
             ind += '  '
             if self.stage:
                 b.append(ind + 'st.sync();')
