@@ -3,8 +3,9 @@
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--impl reference] [--all-configs]
 
 A step is one pass of the whole hot path over one batch of BASELINE.json's size:
-hg_integrate_step = Philox -> RAMBO/Breit-Wigner momenta -> cuts -> |Mbar|^2 -> weight -> (sum w, sum w^2, n_pass),
-fused in one kernel per process; fp64.  Default workload: config 5 (u d~ -> e+ ve g g g, 2^22 events, 2 TeV), the
+hg_integrate_step = Philox -> RAMBO/Breit-Wigner momenta -> cuts -> |Mbar|^2 -> weight -> (sum w, sum w^2, n_pass);
+one fused kernel for configs 1-3, a phase-space kernel and a |M|^2 + reduction kernel per 2^20-event chunk for
+configs 4-5; fp64.  Default workload: config 5 (u d~ -> e+ ve g g g, 2^22 events, 2 TeV), the
 largest one, which is also the config that asks for the BASES-style accumulation.  `value` counts ALL generated
 events per second (events failing the cuts are generated, tested and counted, their matrix element is skipped,
 PAPER.md:1168); the pass fraction is reported.  `e2e` is hg_matrix_element_host: momenta in pinned HOST memory ->
@@ -202,6 +203,7 @@ def run_gpu(args):
     if world > 1:
         dist.init_process_group('nccl', device_id=torch.device('cuda', local))
     ctx = api.Context(local)
+    ctx.hg_set_profiling(True)
     cfg, rs = args.config, SQRT_S[args.config]
     n = args.events or N_EVENTS[cfg]
     info = api.hg_process_info(cfg)
@@ -228,12 +230,18 @@ def run_gpu(args):
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record()
     per_step = []
+    ps_ms = me_ms = 0.0
+    launches = 0
     for _ in range(args.steps):
         a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         a.record()
         acc = step()
         b.record()
         per_step.append((a, b))
+        t_ps, t_me, nl = ctx.hg_last_step_info()   # CUDA events recorded by the library around its kernels
+        ps_ms += t_ps
+        me_ms += t_me
+        launches += nl
     e1.record()
     sync()
     t1 = time.time()
@@ -269,20 +277,28 @@ def run_gpu(args):
            'what': 'hg_matrix_element_host: pinned host momenta -> H2D -> |Mbar|^2 kernel -> D2H, per step'}
     del hp, hme
 
-    flops_step = info['flops_f64'] * acc[3] / world + info['flops_ps'] * n if world > 1 else \
-        info['flops_f64'] * acc[3] + info['flops_ps'] * n
-    achieved = flops_step / (kern_ms * 1e-3) / 1e12
+    n_pass = acc[3] / world if world > 1 else acc[3]
+    staged = ps_ms > 0.0          # two-kernel step (configs 4, 5): the dominant kernel is me_acc_kernel
+    n_chunks = max(1, (launches // args.steps - 1) // 2) if staged else 1
+    me_ms_step = me_ms / args.steps                      # all launches of the dominant kernel in one step
+    flops_kernel = info['flops_f64'] * n_pass + (0.0 if staged else info['flops_ps'] * n)
+    achieved = flops_kernel / (me_ms_step * 1e-3) / 1e12
     traffic = None
     tpath = os.path.join(ROOT, 'profiles', 'roofline_traffic.json')
     if os.path.exists(tpath):
-        traffic = json.load(open(tpath)).get('integrate_cfg%d_%s' % (cfg, pname))
-    roofline = {'bound': 'alu', 'kernel': 'integrate_kernel<P%d,%s>' % (cfg, 'double' if pname == 'f64' else 'float'),
+        traffic = json.load(open(tpath)).get('cfg%d_%s' % (cfg, pname))
+    tname = 'double' if pname == 'f64' else 'float'
+    roofline = {'bound': 'alu',
+                'kernel': ('me_acc_kernel<P%d,%s>' if staged else 'integrate_kernel<P%d,%s>') % (cfg, tname),
                 'achieved': achieved, 'peak': PEAK_NOMINAL_TFLOPS[pname], 'unit': 'TFLOP/s',
                 'frac': achieved / PEAK_NOMINAL_TFLOPS[pname], 'traffic': traffic,
                 'peak_kind': 'nominal non-tensor %s peak (148 SM x %d lanes x 2 x 1.965 GHz, DESIGN.md); '
                              'MEASURED_PEAKS.json has no ALU figure' % (pname, 64 if pname == 'f64' else 128),
                 'peak_measured_fma_chain': peaks[pname], 'frac_of_measured_fma_chain': achieved / peaks[pname],
-                'algorithmic_flops_per_launch': flops_step, 'kernel_ms': kern_ms}
+                'launches_per_step': n_chunks, 'algorithmic_flops_per_launch': flops_kernel / n_chunks,
+                'launch_ms': me_ms_step / n_chunks, 'kernel_ms_per_step': me_ms_step,
+                'phase_space_ms_per_step': ps_ms / args.steps, 'share_of_step': me_ms_step / kern_ms,
+                'flops_per_event': info['flops_f64']}
 
     per_config = {}
     if not args.no_table:
@@ -298,11 +314,14 @@ def run_gpu(args):
             'warmup': max(args.warmup, 3), 'ms_per_step': ms_per_step, 'higher_is_better': True, 'scaling': 'weak',
             'vs_baseline': None, 'dtype': pname, 'data': 'synthetic',
             'config': {'workload': workload_name(cfg, n), 'events_per_gpu': n,
-                       'step': 'hg_integrate_step (Philox -> RAMBO -> cuts -> |M|^2 -> weight -> sums, one fused kernel)',
-                       'l2': 'fused step reads no input from HBM; e2e / matrix_element inputs (%d MB) exceed the 126 MB L2'
-                             % (n * 4 * info['n_ext'] * el >> 20),
+                       'step': 'hg_integrate_step: Philox -> RAMBO -> cuts -> |M|^2 -> weight -> sums; ' + (
+                           'per chunk of 2^20 events a phase-space kernel and a |M|^2 + reduction kernel' if staged
+                           else 'one fused kernel'),
+                       'l2': 'every step regenerates its events; the chunk buffer (%d MB) and the e2e / matrix_element '
+                             'inputs (%d MB) exceed the 126 MB L2' % (
+                                 min(n, 1 << 20) * (4 * info['n_ext'] * el + 9) >> 20, n * 4 * info['n_ext'] * el >> 20),
                        'pass_fraction': acc[3] / acc[2], 'sigma_pb': s, 'sigma_err_pb': ds},
-            'clocks': clocks, 'e2e': e2e, 'gpu_launches': 2 * args.steps, 'roofline': roofline,
+            'clocks': clocks, 'e2e': e2e, 'gpu_launches': launches, 'roofline': roofline,
             'cpu_baseline': cpu_base, 'fma_peak_measured_tflops': peaks, 'per_config': per_config}
     print(json.dumps(line))
     ctx.close()

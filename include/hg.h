@@ -149,12 +149,21 @@ int hg_matrix_element_host(hg_ctx* ctx, int process, int precision, int64_t n, c
 int hg_accumulate(hg_ctx* ctx, int precision, int64_t n, const void* d_me2, const void* d_wps,
                   const uint8_t* d_pass, double sqrt_s_hat, double acc[4], void* cuda_stream);
 
-/* Steps a1-a10 fused in one kernel: each thread draws its event, builds momenta, applies the cuts,
- * evaluates |Mbar|^2 only if it passes, forms w in pb and the block reduces (sum w, sum w^2, n_pass);
- * nothing per-event touches HBM.  Synchronises the stream; acc (HOST, overwritten) = (sum w, sum w^2, n,
+/* Steps a1-a10 in one call.  Configs 1-3: fused in one kernel -- each thread draws its event, builds momenta,
+ * applies the cuts, evaluates |Mbar|^2 only if it passes, forms w in pb and the block reduces (sum w, sum w^2,
+ * n_pass); nothing per-event touches HBM.  Configs 4-5 (matrix elements staged in shared memory at 8 warps per
+ * SM): per chunk of 2^20 events a phase-space kernel writes the points to a context-owned buffer (grown on
+ * demand, freed by hg_destroy) and a second kernel evaluates |Mbar|^2 and reduces; same results.  Synchronises the stream; acc (HOST, overwritten) = (sum w, sum w^2, n,
  * n_pass).  sigma = acc[0]/acc[2]. */
 int hg_integrate_step(hg_ctx* ctx, int process, int precision, uint64_t seed, uint64_t first_event,
                       int64_t n, double sqrt_s_hat, double acc[4], void* cuda_stream);
+
+/* Measurement helpers for bench.py.  hg_set_profiling(ctx, 1) makes hg_integrate_step record CUDA events on the
+ * launching stream around its kernels; hg_last_step_info then returns, for the last hg_integrate_step of the
+ * context, out[0] = milliseconds spent in phase-space kernels (0 when the step is one fused kernel), out[1] =
+ * milliseconds in the kernel(s) that evaluate the matrix element, out[2] = number of kernels launched. */
+int hg_set_profiling(hg_ctx* ctx, int on);
+int hg_last_step_info(const hg_ctx* ctx, double out[3]);
 
 /* Measured-peak helper for the roofline: runs a register-resident FMA chain on every SM
  * and returns the achieved FLOP/s for the given precision in *flops_per_s.  Synchronises. */

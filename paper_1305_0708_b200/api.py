@@ -17,7 +17,7 @@ HG_OK, HG_EINVAL, HG_ENOPROC, HG_ECUDA, HG_ENOTSET = 0, -1, -2, -3, -4
 # symbols include/hg.h declares (checked by tests/test_abi.py)
 SYMBOLS = ('hg_create', 'hg_destroy', 'hg_last_error', 'hg_default_params', 'hg_default_cuts', 'hg_process_info',
            'hg_set_params', 'hg_gen_phase_space', 'hg_matrix_element', 'hg_matrix_element_host', 'hg_accumulate',
-           'hg_integrate_step', 'hg_measure_fma_peak')
+           'hg_integrate_step', 'hg_set_profiling', 'hg_last_step_info', 'hg_measure_fma_peak')
 
 
 class hg_params(C.Structure):
@@ -74,6 +74,8 @@ def load():
     L.hg_accumulate.argtypes = [vp, i32, i64, vp, vp, vp, dbl, C.POINTER(dbl), vp]
     L.hg_integrate_step.argtypes = [vp, i32, i32, u64, u64, i64, dbl, C.POINTER(dbl), vp]
     L.hg_measure_fma_peak.argtypes = [vp, i32, C.POINTER(dbl), vp]
+    L.hg_set_profiling.argtypes = [vp, i32]
+    L.hg_last_step_info.argtypes = [vp, C.POINTER(dbl)]
     _LIB = L
     return L
 
@@ -212,6 +214,15 @@ class Context:
         self._check(self._L.hg_integrate_step(self._h, process, precision, seed, first_event, n, sqrt_s_hat, acc,
                                               _stream(stream)))
         return tuple(acc)
+
+    def hg_set_profiling(self, on):
+        self._check(self._L.hg_set_profiling(self._h, 1 if on else 0))
+
+    def hg_last_step_info(self):
+        """(ms in phase-space kernels, ms in matrix-element kernels, kernels launched) of the last step."""
+        out = (C.c_double * 3)()
+        self._check(self._L.hg_last_step_info(self._h, out))
+        return out[0], out[1], int(out[2])
 
     def hg_measure_fma_peak(self, precision, stream=None):
         out = C.c_double()

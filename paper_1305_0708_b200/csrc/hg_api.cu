@@ -5,6 +5,7 @@
 #include <string.h>
 
 #include <string>
+#include <vector>
 
 #include "hg_couplings.h"
 #include "hg_host_setup.h"
@@ -42,6 +43,10 @@ struct hg_ctx {
   size_t stage_bytes = 0;
   void* d_scratch = nullptr;     // phase-space points of one chunk of hg_integrate_step (staged processes)
   size_t scratch_bytes = 0;
+  int profiling = 0;             // hg_set_profiling
+  std::vector<cudaEvent_t> ev;   // 3 per chunk
+  double t_ps_ms = 0, t_me_ms = 0;
+  int n_launches = 0;            // kernels launched by the last hg_integrate_step
   std::string err;
 };
 
@@ -193,6 +198,7 @@ void hg_destroy(hg_ctx* ctx) {
   if (ctx->h_acc) cudaFreeHost(ctx->h_acc);
   if (ctx->d_stage) cudaFree(ctx->d_stage);
   if (ctx->d_scratch) cudaFree(ctx->d_scratch);
+  for (cudaEvent_t ev : ctx->ev) cudaEventDestroy(ev);
   delete ctx;
 }
 
@@ -418,10 +424,50 @@ int hg_integrate_step(hg_ctx* ctx, int process, int precision, uint64_t seed, ui
       ctx->scratch_bytes = bytes;
     }
   }
+  const int nchunks = per_event ? (int)((n + chunk - 1) / chunk) : 1;
+  cudaEvent_t* ev = nullptr;
+  if (ctx->profiling) {
+    while ((int)ctx->ev.size() < 3 * nchunks) {
+      cudaEvent_t x;
+      if ((e = cudaEventCreate(&x)) != cudaSuccess) return fail_cuda(ctx, e, "hg_integrate_step: cudaEventCreate");
+      ctx->ev.push_back(x);
+    }
+    ev = ctx->ev.data();
+  }
   e = vt->integrate(precision, n, k, seed, first_event, ctx->coup, wscale, ctx->d_partials, nblocks, ctx->d_scratch,
-                    chunk, s);
+                    chunk, ev, s);
   if (e != cudaSuccess) return fail_cuda(ctx, e, "hg_integrate_step");
-  return finish(ctx, nblocks, n, acc, s, "hg_integrate_step");
+  ctx->n_launches = (per_event ? 2 * nchunks : 1) + 1;
+  rc = finish(ctx, nblocks, n, acc, s, "hg_integrate_step");  // synchronises the stream
+  if (rc == HG_OK && ev) {
+    ctx->t_ps_ms = ctx->t_me_ms = 0;
+    for (int i = 0; i < nchunks; ++i) {
+      float a = 0, b = 0;
+      if (per_event) {
+        cudaEventElapsedTime(&a, ev[3 * i], ev[3 * i + 1]);
+        cudaEventElapsedTime(&b, ev[3 * i + 1], ev[3 * i + 2]);
+      } else {
+        cudaEventElapsedTime(&b, ev[0], ev[2]);
+      }
+      ctx->t_ps_ms += a;
+      ctx->t_me_ms += b;
+    }
+  }
+  return rc;
+}
+
+int hg_set_profiling(hg_ctx* ctx, int on) {
+  if (!ctx) return HG_EINVAL;
+  ctx->profiling = on ? 1 : 0;
+  return HG_OK;
+}
+
+int hg_last_step_info(const hg_ctx* ctx, double out[3]) {
+  if (!ctx || !out) return HG_EINVAL;
+  out[0] = ctx->t_ps_ms;
+  out[1] = ctx->t_me_ms;
+  out[2] = (double)ctx->n_launches;
+  return HG_OK;
 }
 
 int hg_measure_fma_peak(hg_ctx* ctx, int precision, double* flops_per_s, void* cuda_stream) {

@@ -24,11 +24,13 @@ struct ProcVTable {
   cudaError_t (*ps)(int prec, int64_t n, const PsConst& k, uint64_t seed, uint64_t first, void* d_p,
                     void* d_wps, uint8_t* d_pass, cudaStream_t s);
   // hg_integrate_step: writes nblocks x (sum w, sum w^2, n_pass) partials; wscale = (hbar c)^2 / (2 s_hat)
+  // ev (or NULL): 3 events per chunk, recorded on s before the phase-space kernel, between the two kernels and
+  // after the matrix-element kernel (hg_set_profiling); a fused process records ev[0] and ev[2] around its kernel.
   // Staged processes (scratch_bytes_per_event > 0) run the step as two kernels per chunk of `chunk` events
   // through the caller's scratch buffer (momenta, weight, pass flag); the others ignore scratch and chunk.
   cudaError_t (*integrate)(int prec, int64_t n, const PsConst& k, uint64_t seed, uint64_t first,
                            const Coup<double>& c, double wscale, double* d_partials, int nblocks,
-                           void* d_scratch, int64_t chunk, cudaStream_t s);
+                           void* d_scratch, int64_t chunk, cudaEvent_t* ev, cudaStream_t s);
   // resident blocks per SM of the fused kernel for this precision (occupancy query)
   cudaError_t (*int_blocks_per_sm)(int prec, int* out);
   // bytes of scratch per event of a chunk for the given precision (0: the step is one fused kernel)

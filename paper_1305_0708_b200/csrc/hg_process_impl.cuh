@@ -243,11 +243,13 @@ struct Launch {
   template <class T>
   static cudaError_t integrate_t(int64_t n, const PsConst& k, uint64_t seed, uint64_t first, const Coup<T>& c,
                                  double wscale, double* d_partials, int nblocks, void* d_scratch, int64_t chunk,
-                                 cudaStream_t s) {
+                                 cudaEvent_t* ev, cudaStream_t s) {
     constexpr int TH = int_thr<T>();
     constexpr size_t smem = stage_bytes<P, T, TH>();
     if constexpr (P::n_stage == 0) {
+      if (ev) cudaEventRecord(ev[0], s);
       integrate_kernel<P, T, TH><<<nblocks, TH, smem, s>>>(k, seed, first, n, c, wscale, d_partials);
+      if (ev) cudaEventRecord(ev[2], s);
       return cudaGetLastError();
     } else {
       cudaError_t err = allow_smem(me_acc_kernel<P, T, TH>, smem);
@@ -257,10 +259,14 @@ struct Launch {
         T* d_p = (T*)d_scratch;                                      // [n_ext][4][m]
         double* d_w = (double*)((char*)d_scratch + scratch_p_bytes<T>(chunk));
         uint8_t* d_ok = (uint8_t*)(d_w + chunk);
+        cudaEvent_t* e3 = ev ? ev + 3 * (off / chunk) : nullptr;
+        if (e3) cudaEventRecord(e3[0], s);
         ps_kernel<P, T, double><<<(unsigned)((m + 127) / 128), 128, 0, s>>>(k, seed, first + (uint64_t)off, m, d_p,
                                                                             d_w, d_ok);
+        if (e3) cudaEventRecord(e3[1], s);
         me_acc_kernel<P, T, TH><<<nblocks, TH, smem, s>>>(d_p, d_w, d_ok, m, c, wscale, off > 0 ? 1 : 0,
                                                           d_partials);
+        if (e3) cudaEventRecord(e3[2], s);
       }
       return cudaGetLastError();
     }
@@ -275,11 +281,11 @@ struct Launch {
   }
   static cudaError_t integrate(int prec, int64_t n, const PsConst& k, uint64_t seed, uint64_t first,
                                const Coup<double>& c, double wscale, double* d_partials, int nblocks,
-                               void* d_scratch, int64_t chunk, cudaStream_t s) {
+                               void* d_scratch, int64_t chunk, cudaEvent_t* ev, cudaStream_t s) {
     if (prec == HG_F64)
-      return integrate_t<double>(n, k, seed, first, c, wscale, d_partials, nblocks, d_scratch, chunk, s);
+      return integrate_t<double>(n, k, seed, first, c, wscale, d_partials, nblocks, d_scratch, chunk, ev, s);
     return integrate_t<float>(n, k, seed, first, coup_cast<float>(c), wscale, d_partials, nblocks, d_scratch, chunk,
-                              s);
+                              ev, s);
   }
   template <class T>
   static cudaError_t int_blocks_t(int* out) {
