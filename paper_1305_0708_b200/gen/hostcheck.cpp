@@ -1,0 +1,47 @@
+// hostcheck.cpp -- build-time / test tool of the generator: evaluates the generated matrix elements in fp64 on the
+// HOST (the device library compiles as plain C++) for momenta read from stdin, so that the emitted code can be
+// checked without a GPU (tests/test_generated_host.py).  Never linked into libhg.so.
+//   input : lines "pid  E px py pz  E px py pz ..." (n_ext momenta, leg order of include/hg.h)
+//   output: one line per input line, |Mbar|^2 with 17 significant digits
+#include <stdio.h>
+
+#include "flopcount.h"
+#include "../csrc/hg_couplings.h"
+#include "../csrc/hg_host_setup.h"
+#include "../csrc/generated/hg_proc_1.cuh"
+#include "../csrc/generated/hg_proc_2.cuh"
+#include "../csrc/generated/hg_proc_3.cuh"
+#include "../csrc/generated/hg_proc_4.cuh"
+#include "../csrc/generated/hg_proc_5.cuh"
+
+using namespace hg;
+
+template <class P>
+bool eval(const Coup<double>& c) {
+  Mom<double> p[P::n_ext];
+  for (int l = 0; l < P::n_ext; ++l)
+    if (scanf("%lf %lf %lf %lf", &p[l].e, &p[l].x, &p[l].y, &p[l].z) != 4) return false;
+  static double area[P::n_stage + 1];
+  const HostStage<double> st{area};
+  printf("%.17g\n", P::template me2<double>(p, c, st));
+  return true;
+}
+
+int main() {
+  hg_params par;
+  default_params(&par);
+  const Coup<double> c = derive_couplings(par);
+  int pid;
+  while (scanf("%d", &pid) == 1) {
+    bool ok = false;
+    switch (pid) {
+      case 1: ok = eval<P1>(c); break;
+      case 2: ok = eval<P2>(c); break;
+      case 3: ok = eval<P3>(c); break;
+      case 4: ok = eval<P4>(c); break;
+      case 5: ok = eval<P5>(c); break;
+    }
+    if (!ok) return 1;
+  }
+  return 0;
+}
