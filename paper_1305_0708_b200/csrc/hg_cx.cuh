@@ -147,6 +147,44 @@ struct Sp {  // Dirac spinor in the chiral representation: slots A = c[0],c[1]; 
   cx<T> c[4];
 };
 
+// sums of wavefunctions (merged currents of the generator)
+template <class T>
+HG_HD Vc<T> operator+(const Vc<T>& a, const Vc<T>& b) {
+  Vc<T> r;
+  for (int i = 0; i < 4; ++i) r.c[i] = a.c[i] + b.c[i];
+  return r;
+}
+template <class T>
+HG_HD Vc<T> operator-(const Vc<T>& a, const Vc<T>& b) {
+  Vc<T> r;
+  for (int i = 0; i < 4; ++i) r.c[i] = a.c[i] - b.c[i];
+  return r;
+}
+template <class T>
+HG_HD Vc<T> operator-(const Vc<T>& a) {
+  Vc<T> r;
+  for (int i = 0; i < 4; ++i) r.c[i] = -a.c[i];
+  return r;
+}
+template <class T>
+HG_HD Sp<T> operator+(const Sp<T>& a, const Sp<T>& b) {
+  Sp<T> r;
+  for (int i = 0; i < 4; ++i) r.c[i] = a.c[i] + b.c[i];
+  return r;
+}
+template <class T>
+HG_HD Sp<T> operator-(const Sp<T>& a, const Sp<T>& b) {
+  Sp<T> r;
+  for (int i = 0; i < 4; ++i) r.c[i] = a.c[i] - b.c[i];
+  return r;
+}
+template <class T>
+HG_HD Sp<T> operator-(const Sp<T>& a) {
+  Sp<T> r;
+  for (int i = 0; i < 4; ++i) r.c[i] = -a.c[i];
+  return r;
+}
+
 // Minkowski products (no complex conjugation)
 template <class T>
 HG_HD cx<T> vdot(const Vc<T>& a, const Vc<T>& b) {

@@ -41,10 +41,16 @@ class Node:
     struct: int = 0           # 1..3 for the colour structures of a four-gluon vertex
     colour: object = None
     leg: int = -1             # leaf only
+    members: tuple = ()       # sum node: the currents added up (= children), with relative signs msigns
+    msigns: tuple = ()
 
     @property
     def is_leaf(self):
-        return self.vertex is None
+        return self.vertex is None and not self.members
+
+    @property
+    def is_sum(self):
+        return bool(self.members)
 
     @property
     def particle(self):
@@ -126,8 +132,13 @@ def _match(vertex, fields):
 
 
 class Diagrams:
-    def __init__(self, spec):
+    def __init__(self, spec, merge=False):
+        """merge=True: off-shell currents over the same legs with the same field and the same colour structure (up
+        to a sign) are added into one current before they are used -- by linearity every vertex that would be
+        evaluated once per member is evaluated once for the sum (e.g. the W emitted before or after a gluon on the
+        quark line).  The amplitude is unchanged; the diagram COUNTS are those of the unmerged enumeration."""
         self.spec = spec
+        self.merge = merge
         self.legs = []
         for nm in spec.initial:
             self.legs.append(Leg(len(self.legs), nm, 'in', nm))
@@ -151,6 +162,33 @@ class Diagrams:
             if (mask == d or comp == d) and fld not in (nm, anti(nm)):
                 return False
         return True
+
+    def _merge(self, m, nodes):
+        groups = {}
+        for nd in nodes:
+            key = (nd.field, nd.colour.kind, frozenset(nd.colour.terms))
+            groups.setdefault(key, []).append(nd)
+        out = []
+        for key, grp in groups.items():
+            # split the group into classes of proportional colour (ratio +-1)
+            classes = []
+            for nd in grp:
+                for cl in classes:
+                    ref = cl[0][0].colour.terms
+                    ratios = {nd.colour.terms[w] / ref[w] for w in ref}
+                    if len(ratios) == 1 and abs(next(iter(ratios))) == 1:
+                        cl.append((nd, int(next(iter(ratios)))))
+                        break
+                else:
+                    classes.append([(nd, 1)])
+            for cl in classes:
+                if len(cl) == 1:
+                    out.append(cl[0][0])
+                else:
+                    mem = tuple(nd for nd, _ in cl)
+                    out.append(self._new_node(mask=m, field=mem[0].field, children=mem, members=mem,
+                                              msigns=tuple(sg for _, sg in cl), colour=mem[0].colour))
+        return out
 
     def _new_node(self, **kw):
         nd = Node(uid=self._uid, **kw)
@@ -236,6 +274,8 @@ class Diagrams:
                                     res.append(self._new_node(mask=m, field=out_field, vertex=v, children=combo,
                                                               slots=slots, out_slot=free[0], struct=struct,
                                                               colour=col))
+            if self.merge and len(res) > 1:
+                res = self._merge(m, res)
             memo[m] = res
             return res
 

@@ -79,6 +79,10 @@ class Emitter:
             return memo[key]
         if nd.is_leaf:
             r = self._leaf_mask(nd, hel)
+        elif nd.is_sum:
+            r = 0
+            for ch in nd.members:
+                r |= self._node_mask(ch, hel, memo)
         else:
             cm = [self._node_mask(ch, hel, memo) for ch in nd.children]
             if 0 in cm:
@@ -403,6 +407,16 @@ class CodeGen(Emitter):
             return '%s<T>(p[%d], %d, %d)' % (fn, nd.leg, hel[nd.leg], self._nsf(lg))
         raise NotImplementedError
 
+    def _sum_expr(self, nd, vi, hel):
+        """Sum of the member currents that do not vanish for this helicity assignment."""
+        txt = ''
+        for ch, sg in zip(nd.members, nd.msigns):
+            if self._node_mask(ch, hel, self.memo) == 0:
+                continue
+            r = self._ref(self._name(ch, vi, hel))
+            txt += (' + ' if sg > 0 else ' - ') + r if txt else ('-' if sg < 0 else '') + r
+        return txt
+
     def _node_expr(self, nd, vi, hel):
         v = nd.vertex
         by_slot = dict(zip(nd.slots, nd.children))
@@ -529,7 +543,12 @@ class CodeGen(Emitter):
                 need(ch)
             self._reg(name, self._wtype_decl(nd), dep, mask=self._node_mask(nd, hel, self.memo))
             self._begin(dep)
-            expr = self._leaf_expr(nd, hel) if nd.is_leaf else self._node_expr(nd, vi, hel)
+            if nd.is_leaf:
+                expr = self._leaf_expr(nd, hel)
+            elif nd.is_sum:
+                expr = self._sum_expr(nd, vi, hel)
+            else:
+                expr = self._node_expr(nd, vi, hel)
             item = ('def', name, expr, self.cur_loads)
             if dep == 0:
                 self.shared[name] = True
