@@ -238,6 +238,32 @@ def test_full_size_sampled_outputs_and_cross_section(ctx, api, cfg):
     assert abs(s32 - s) <= 1e-4 * s and acc32[3] == acc[3]
 
 
+@pytest.mark.parametrize('cfg', [3, 5])
+def test_smallest_invariants_edge_stress(ctx, api, cfg):
+    """Edge stress (SURVEY.md 8c parity protocol): of 2^20 device-generated points, the passing events with the
+    smallest min(s_ij) over all pairs of massless legs (closest to the soft / collinear edges the cuts leave),
+    fp64 against the oracle at the device's own momenta, and fp32 within its 99.9th-percentile bound."""
+    n, rs = 1 << 20, opr.SQRT_S[cfg]
+    p, wps, ok = ctx.hg_gen_phase_space(cfg, api.HG_F64, SEED, 0, n, rs)
+    next_ = p.shape[0]
+    smin = torch.full((n,), float('inf'), dtype=torch.float64, device=p.device)
+    for a in range(next_):
+        for b in range(a + 1, next_):
+            d = p[a, 0] * p[b, 0] - p[a, 1] * p[b, 1] - p[a, 2] * p[b, 2] - p[a, 3] * p[b, 3]
+            smin = torch.minimum(smin, 2 * d.abs())
+    smin = torch.where(ok.bool(), smin, torch.full_like(smin, float('inf')))
+    k = 24 if cfg == 3 else 8
+    idx = torch.topk(smin, k, largest=False).indices
+    me = ctx.hg_matrix_element(cfg, api.HG_F64, p)
+    me32 = ctx.hg_matrix_element(cfg, api.HG_F32, p.float())
+    pd = p[:, :, idx].cpu().numpy().transpose(2, 0, 1)
+    ref = opr.me2(opr.config(cfg), pd, PAR)
+    got = me[idx].cpu().numpy()
+    got32 = me32[idx].cpu().numpy().astype(np.float64)
+    assert np.all(np.abs(got - ref) <= 1e-11 * ref), (cfg, float((np.abs(got - ref) / ref).max()))
+    assert np.all(np.abs(got32 - ref) <= 1e-3 * ref), (cfg, float((np.abs(got32 - ref) / ref).max()))
+
+
 def test_edge_cases_and_errors(ctx, api):
     from paper_1305_0708_b200.api import HgError
     # empty batches are successful no-ops
