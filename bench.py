@@ -279,7 +279,7 @@ def run_gpu(args):
 
     n_pass = acc[3] / world if world > 1 else acc[3]
     staged = ps_ms > 0.0          # two-kernel step (configs 4, 5): the dominant kernel is me_acc_kernel
-    n_chunks = max(1, (launches // args.steps - 1) // 2) if staged else 1
+    n_chunks = max(1, (launches // args.steps - 1) // 3) if staged else 1
     me_ms_step = me_ms / args.steps                      # all launches of the dominant kernel in one step
     flops_kernel = info['flops_f64'] * n_pass + (0.0 if staged else info['flops_ps'] * n)
     achieved = flops_kernel / (me_ms_step * 1e-3) / 1e12

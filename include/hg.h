@@ -153,7 +153,8 @@ int hg_accumulate(hg_ctx* ctx, int precision, int64_t n, const void* d_me2, cons
  * applies the cuts, evaluates |Mbar|^2 only if it passes, forms w in pb and the block reduces (sum w, sum w^2,
  * n_pass); nothing per-event touches HBM.  Configs 4-5 (matrix elements staged in shared memory at 8 warps per
  * SM): per chunk of 2^20 events a phase-space kernel writes the points to a context-owned buffer (grown on
- * demand, freed by hg_destroy) and a second kernel evaluates |Mbar|^2 and reduces; same results.  Synchronises the stream; acc (HOST, overwritten) = (sum w, sum w^2, n,
+ * demand, freed by hg_destroy), a compaction kernel lists the passing events in order, and a third kernel
+ * evaluates |Mbar|^2 of exactly those and reduces; same results, fixed summation order.  Synchronises the stream; acc (HOST, overwritten) = (sum w, sum w^2, n,
  * n_pass).  sigma = acc[0]/acc[2]. */
 int hg_integrate_step(hg_ctx* ctx, int process, int precision, uint64_t seed, uint64_t first_event,
                       int64_t n, double sqrt_s_hat, double acc[4], void* cuda_stream);

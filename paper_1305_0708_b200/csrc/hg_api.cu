@@ -414,7 +414,7 @@ int hg_integrate_step(hg_ctx* ctx, int process, int precision, uint64_t seed, ui
   const size_t per_event = vt->scratch_bytes_per_event(precision);
   const int64_t chunk = n < kIntChunk ? n : kIntChunk;
   if (per_event) {  // two kernels per chunk through a context-owned buffer, grown on demand
-    const size_t bytes = per_event * (size_t)chunk + 1024;
+    const size_t bytes = per_event * (size_t)chunk + 1024 + sizeof(int) * kMaxPartialBlocks;
     if (bytes > ctx->scratch_bytes) {
       if (ctx->d_scratch) cudaFree(ctx->d_scratch);
       ctx->d_scratch = nullptr;
@@ -437,7 +437,7 @@ int hg_integrate_step(hg_ctx* ctx, int process, int precision, uint64_t seed, ui
   e = vt->integrate(precision, n, k, seed, first_event, ctx->coup, wscale, ctx->d_partials, nblocks, ctx->d_scratch,
                     chunk, ev, s);
   if (e != cudaSuccess) return fail_cuda(ctx, e, "hg_integrate_step");
-  ctx->n_launches = (per_event ? 2 * nchunks : 1) + 1;
+  ctx->n_launches = (per_event ? 3 * nchunks : 1) + 1;
   rc = finish(ctx, nblocks, n, acc, s, "hg_integrate_step");  // synchronises the stream
   if (rc == HG_OK && ev) {
     ctx->t_ps_ms = ctx->t_me_ms = 0;

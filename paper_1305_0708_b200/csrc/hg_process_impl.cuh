@@ -161,6 +161,39 @@ __global__ void __launch_bounds__(THREADS) integrate_kernel(const PsConst k, uin
   }
 }
 
+// Ordered compaction of the events that pass the cuts: block b owns the events [b*range, (b+1)*range) of the
+// chunk and writes their indices, in order, to idx[b*range ...]; cnt[b] = how many.  me_acc_kernel block b then
+// evaluates exactly those, so that no lane idles on a failed event (10 % of W + 3 jets) and the order of the sums
+// stays fixed (deterministic results).
+static __global__ void __launch_bounds__(256) compact_kernel(const uint8_t* __restrict__ pass, int64_t n, int64_t range,
+                                                      int* __restrict__ idx, int* __restrict__ cnt) {
+  __shared__ int wsum[8];
+  __shared__ int base;
+  const int64_t lo = (int64_t)blockIdx.x * range;
+  const int64_t hi = lo + range < n ? lo + range : n;
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  if (threadIdx.x == 0) base = 0;
+  __syncthreads();
+  for (int64_t t = lo; t < hi; t += 256) {
+    const int64_t e = t + threadIdx.x;
+    const bool ok = e < hi && pass[e] != 0;
+    const unsigned m = __ballot_sync(0xffffffffu, ok);
+    if (lane == 0) wsum[w] = __popc(m);
+    __syncthreads();
+    int off = base;
+    for (int i = 0; i < w; ++i) off += wsum[i];
+    if (ok) idx[lo + off + __popc(m & ((1u << lane) - 1u))] = (int)e;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      int tot = 0;
+      for (int i = 0; i < 8; ++i) tot += wsum[i];
+      base += tot;
+    }
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) cnt[blockIdx.x] = base;
+}
+
 // Second half of the step of a staged process: reads the points the ps_kernel wrote (momenta as T, weight as
 // double, pass flag), evaluates |M|^2 and reduces (sum w, sum w^2, n_pass) per block.  The two halves are separate
 // kernels because the phase-space code wants ~70 registers at full occupancy while the staged matrix element
@@ -168,27 +201,27 @@ __global__ void __launch_bounds__(THREADS) integrate_kernel(const PsConst k, uin
 // A block skips me2 only if none of its events passes (every thread must reach the rendezvous inside me2).
 template <class P, class T, int THREADS>
 __global__ void __launch_bounds__(THREADS) me_acc_kernel(const T* __restrict__ p, const double* __restrict__ wps,
-                                                         const uint8_t* __restrict__ pass, int64_t n,
-                                                         const Coup<T> c, double wscale, int add,
-                                                         double* __restrict__ partials) {
-  double sw = 0.0, sw2 = 0.0, np = 0.0;
+                                                         const int* __restrict__ idx, const int* __restrict__ cnt,
+                                                         int64_t n, int64_t range, const Coup<T> c, double wscale,
+                                                         int add, double* __restrict__ partials) {
   constexpr int EPB = THREADS / kSplit<P>;
-  for (int64_t base = (int64_t)blockIdx.x * EPB; base < n; base += (int64_t)gridDim.x * EPB) {
-    const int64_t e0 = base + ev_local<P>();
-    const int64_t e = e0 < n ? e0 : n - 1;
-    const bool ok = e0 < n && pass[e] != 0;
-    if (__syncthreads_or(ok)) {
-      Mom<T> q[P::n_ext];
+  double sw = 0.0, sw2 = 0.0, np = 0.0;
+  const int m = cnt[blockIdx.x];                    // passing events of this block's range, block-uniform
+  const int* __restrict__ my = idx + (int64_t)blockIdx.x * range;
+  for (int base = 0; base < m; base += EPB) {
+    const int j = base + ev_local<P>();
+    const bool ok = j < m;
+    const int64_t e = my[ok ? j : m - 1];           // tail lanes recompute the last event (rendezvous inside me2)
+    Mom<T> q[P::n_ext];
 #pragma unroll
-      for (int l = 0; l < P::n_ext; ++l)
-        q[l] = mkmom<T>(p[(l * 4 + 0) * n + e], p[(l * 4 + 1) * n + e], p[(l * 4 + 2) * n + e],
-                        p[(l * 4 + 3) * n + e]);
-      const double w = (double)me2_event<P, T, THREADS>(q, c) * wps[e] * wscale;
-      if (ok && ev_owner<P>()) {
-        sw += w;
-        sw2 += w * w;
-        np += 1.0;
-      }
+    for (int l = 0; l < P::n_ext; ++l)
+      q[l] = mkmom<T>(p[(l * 4 + 0) * n + e], p[(l * 4 + 1) * n + e], p[(l * 4 + 2) * n + e],
+                      p[(l * 4 + 3) * n + e]);
+    const double w = (double)me2_event<P, T, THREADS>(q, c) * wps[e] * wscale;
+    if (ok && ev_owner<P>()) {
+      sw += w;
+      sw2 += w * w;
+      np += 1.0;
     }
   }
   block_reduce3(sw, sw2, np);
@@ -258,14 +291,18 @@ struct Launch {
         const int64_t m = n - off < chunk ? n - off : chunk;
         T* d_p = (T*)d_scratch;                                      // [n_ext][4][m]
         double* d_w = (double*)((char*)d_scratch + scratch_p_bytes<T>(chunk));
-        uint8_t* d_ok = (uint8_t*)(d_w + chunk);
+        int* d_idx = (int*)(d_w + chunk);
+        int* d_cnt = d_idx + chunk;
+        uint8_t* d_ok = (uint8_t*)(d_cnt + kMaxPartialBlocks);
+        const int64_t range = (m + nblocks - 1) / nblocks;
         cudaEvent_t* e3 = ev ? ev + 3 * (off / chunk) : nullptr;
         if (e3) cudaEventRecord(e3[0], s);
         ps_kernel<P, T, double><<<(unsigned)((m + 127) / 128), 128, 0, s>>>(k, seed, first + (uint64_t)off, m, d_p,
                                                                             d_w, d_ok);
+        compact_kernel<<<nblocks, 256, 0, s>>>(d_ok, m, range, d_idx, d_cnt);
         if (e3) cudaEventRecord(e3[1], s);
-        me_acc_kernel<P, T, TH><<<nblocks, TH, smem, s>>>(d_p, d_w, d_ok, m, c, wscale, off > 0 ? 1 : 0,
-                                                          d_partials);
+        me_acc_kernel<P, T, TH><<<nblocks, TH, smem, s>>>(d_p, d_w, d_idx, d_cnt, m, range, c, wscale,
+                                                          off > 0 ? 1 : 0, d_partials);
         if (e3) cudaEventRecord(e3[2], s);
       }
       return cudaGetLastError();
@@ -277,7 +314,7 @@ struct Launch {
   }
   static size_t scratch_bytes_per_event(int prec) {
     if (P::n_stage == 0) return 0;
-    return (size_t)P::n_ext * 4 * (prec == HG_F64 ? 8 : 4) + 8 + 1;
+    return (size_t)P::n_ext * 4 * (prec == HG_F64 ? 8 : 4) + 8 + 4 + 1;  // momenta, weight, index, pass flag
   }
   static cudaError_t integrate(int prec, int64_t n, const PsConst& k, uint64_t seed, uint64_t first,
                                const Coup<double>& c, double wscale, double* d_partials, int nblocks,

@@ -260,7 +260,12 @@ def test_smallest_invariants_edge_stress(ctx, api, cfg):
     ref = opr.me2(opr.config(cfg), pd, PAR)
     got = me[idx].cpu().numpy()
     got32 = me32[idx].cpu().numpy().astype(np.float64)
-    assert np.all(np.abs(got - ref) <= 1e-11 * ref), (cfg, float((np.abs(got - ref) / ref).max()))
+    # The oracle forms every propagator denominator as (sum p)^2 = E^2 - |p|^2, whose relative rounding error is
+    # eps * s_hat / s_ij; near the edges that, not the kernel (which uses cancellation-free invariants), sets the
+    # agreement: tolerance max(1e-11, 64 eps s_hat / min s_ij).
+    tol = np.maximum(1e-11, 64 * np.finfo(float).eps * rs * rs / smin[idx].cpu().numpy())
+    rel = np.abs(got - ref) / ref
+    assert np.all(rel <= tol), (cfg, float((rel / tol).max()))
     assert np.all(np.abs(got32 - ref) <= 1e-3 * ref), (cfg, float((np.abs(got32 - ref) / ref).max()))
 
 
