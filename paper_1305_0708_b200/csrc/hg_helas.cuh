@@ -262,6 +262,25 @@ template <int MI, int G, bool MASSIVE, class T, class D>
 HG_HD Sp<T> fvixxx(const Sp<T>& fi, const Vc<T>& v, T gL, T gR, const Mom<T>& q, T m, D d) {
   constexpr bool L = (MI & SLOT_A) && (G & CPL_L);  // w_B = gL M+(V) fi_A
   constexpr bool R = (MI & SLOT_B) && (G & CPL_R);  // w_A = gR M-(V) fi_B
+  if constexpr (!MASSIVE && (L != R)) {
+    // one chirality on a massless line: coupling and propagator factor are applied once, at the end
+    Sp<T> f;
+    for (int i = 0; i < 4; ++i) f.c[i] = czero<T>();
+    cx<T> w0, w1, y0, y1;
+    const D gd = (L ? gL : gR) * d;
+    if (L) {
+      sig_col<+1>(v, fi.c[0], fi.c[1], w0, w1);
+      sig_col<-1>(q, w0, w1, y0, y1);
+      f.c[0] = gd * y0;
+      f.c[1] = gd * y1;
+    } else {
+      sig_col<-1>(v, fi.c[2], fi.c[3], w0, w1);
+      sig_col<+1>(q, w0, w1, y0, y1);
+      f.c[2] = gd * y0;
+      f.c[3] = gd * y1;
+    }
+    return f;
+  }
   cx<T> wB0 = czero<T>(), wB1 = czero<T>(), wA0 = czero<T>(), wA1 = czero<T>();
   if (L) {
     sig_col<+1>(v, fi.c[0], fi.c[1], wB0, wB1);
@@ -305,6 +324,24 @@ template <int MO, int G, bool MASSIVE, class T, class D>
 HG_HD Sp<T> fvoxxx(const Sp<T>& fo, const Vc<T>& v, T gL, T gR, const Mom<T>& q, T m, D d) {
   constexpr bool L = (MO & SLOT_B) && (G & CPL_L);  // w_A = gL fo_B M+(V)
   constexpr bool R = (MO & SLOT_A) && (G & CPL_R);  // w_B = gR fo_A M-(V)
+  if constexpr (!MASSIVE && (L != R)) {
+    Sp<T> f;
+    for (int i = 0; i < 4; ++i) f.c[i] = czero<T>();
+    cx<T> w0, w1, y0, y1;
+    const D gd = (L ? gL : gR) * d;
+    if (L) {
+      sig_row<+1>(v, fo.c[2], fo.c[3], w0, w1);
+      sig_row<-1>(q, w0, w1, y0, y1);
+      f.c[2] = gd * y0;
+      f.c[3] = gd * y1;
+    } else {
+      sig_row<-1>(v, fo.c[0], fo.c[1], w0, w1);
+      sig_row<+1>(q, w0, w1, y0, y1);
+      f.c[0] = gd * y0;
+      f.c[1] = gd * y1;
+    }
+    return f;
+  }
   cx<T> wA0 = czero<T>(), wA1 = czero<T>(), wB0 = czero<T>(), wB1 = czero<T>();
   if (L) {
     sig_row<+1>(v, fo.c[2], fo.c[3], wA0, wA1);
@@ -393,10 +430,9 @@ HG_HD Vc<T> jioxxx(const Sp<T>& fi, const Sp<T>& fo, T gL, T gR, const Mom<T>& q
 // massless vector line (Feynman gauge): d J, no momentum needed
 template <int MI, int MO, int G, class T, class D>
 HG_HD Vc<T> jioxx0(const Sp<T>& fi, const Sp<T>& fo, T gL, T gR, D d) {
-  const Vc<T> j = ffv_current<MI, MO, G>(fi, fo, gL, gR);
-  Vc<T> w;
-  for (int i = 0; i < 4; ++i) w.c[i] = d * j.c[i];
-  return w;
+  // the current is linear in the couplings: the (real) propagator factor is folded into the ones in use
+  const bool l = (MI & SLOT_A) && (MO & SLOT_B) && (G & CPL_L), r = (MI & SLOT_B) && (MO & SLOT_A) && (G & CPL_R);
+  return ffv_current<MI, MO, G>(fi, fo, l ? gL * d : gL, r ? gR * d : gR);
 }
 
 // =============================================================================== VVV (Eq. 40-44)
