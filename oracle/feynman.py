@@ -21,10 +21,17 @@ Feynman rules (all momenta incoming at a vertex; derived from the paper's Lagran
   gggg  Eq. 48   -i g_s^2 [ f^{abe}f^{cde}(g^{mu rho}g^{nu sigma}-g^{mu sigma}g^{nu rho})
                                           + f^{ace}f^{bde}(g^{mu nu}g^{rho sigma}-g^{mu sigma}g^{nu rho})
                                           + f^{ade}f^{bce}(g^{mu nu}g^{rho sigma}-g^{mu rho}g^{nu sigma}) ]
+  FFS   Eq. 39   i (gL PL + gR PR)             t t H: gL = gR = -m_t / v
+  VVS   Eq. 50   i g g^{mu nu}                   W W H: g_W m_W,  Z Z H: g_Z m_Z   (v = 2 m_W / g_W)
+  VVSS  Eq. 51   i g g^{mu nu}                   W W H H: g_W^2 / 2,  Z Z H H: g_Z^2 / 2
+  SSS   Eq. 52   i g                             H H H: -3 m_H^2 / v
+        (the coefficients are those of the Feynman rules that follow from |D Phi|^2, the Higgs potential and the
+        Yukawa term with Phi = (0, (v + H)/sqrt2); the scalar wavefunction is 1, Eq. 34)
   propagators (widths PAPER.md:1591, 1637; reading SURVEY 8c-A4):
         fermion  i (pslash + m) / (p^2 - m^2 + i m Gamma)
         massless vector (Feynman gauge)  -i g_{mu nu} / q^2
         massive vector (unitary gauge)   -i (g_{mu nu} - q_mu q_nu / m^2) / (q^2 - m^2 + i m Gamma)
+        scalar   i / (q^2 - m^2 + i m Gamma)
 """
 import itertools
 import numpy as np
@@ -56,6 +63,7 @@ _add('g', 'V', 8, None, None, 'g')
 _add('a', 'V', 1, None, None, 'a')
 _add('z', 'V', 1, 'mz', 'gz', 'z')
 _add('w+', 'V', 1, 'mw', 'gw', 'w-')
+_add('h', 'S', 1, 'mh', 'gh', 'h')
 PARTICLES = {'u', 'd', 't', 'b', 'e-', 'mu-', 've', 'vm'}  # fermion (not anti-fermion) names
 
 
@@ -101,6 +109,7 @@ def build_vertices(par, names):
     """names: iterable of vertex keys, e.g. 'uug', 'udw', 'ggg', 'gggg', 'uua', 'eez' ..."""
     c = sm.couplings(par)
     gs = c['gs']
+    vev = 2.0 * par['mw'] / c['gw']
     out = []
     for n in names:
         if n == 'ggg':
@@ -121,6 +130,19 @@ def build_vertices(par, names):
             gl, gr = c['w']
             out.append(ffv(up, dn, 'w+', gl, gr))  # dn + W+ -> up
             out.append(ffv(dn, up, 'w-', gl, gr))  # up + W- -> dn   (hermitian conjugate, real coupling)
+        elif n == 'tth':
+            y = -par['mt'] / vev
+            out.append(Vertex('FFS', ('t~', 't', 'h'), row='t~', col='t', sca='h', gl=y, gr=y))
+        elif n == 'wwh':
+            out.append(Vertex('VVS', ('w-', 'w+', 'h'), g=c['gw'] * par['mw']))
+        elif n == 'zzh':
+            out.append(Vertex('VVS', ('z', 'z', 'h'), g=c['gz'] * par['mz']))
+        elif n == 'wwhh':
+            out.append(Vertex('VVSS', ('w-', 'w+', 'h', 'h'), g=0.5 * c['gw'] ** 2))
+        elif n == 'zzhh':
+            out.append(Vertex('VVSS', ('z', 'z', 'h', 'h'), g=0.5 * c['gz'] ** 2))
+        elif n == 'hhh':
+            out.append(Vertex('SSS', ('h', 'h', 'h'), g=-3.0 * par['mh'] ** 2 / vev))
         else:
             raise ValueError(n)
     return out
@@ -240,6 +262,10 @@ def _vertex_colour_tensors(v):
     """List of (tensor, axis roles).  FFV axes (row j, col i, vec a); VVV (a,b,c); VVVV (a,b,c,d) x3."""
     if v.kind == 'FFV':
         return [_ffv_colour(v)]
+    if v.kind == 'FFS':
+        return [np.eye(coldim(v.col), dtype=complex)[:, :, None]]
+    if v.kind in ('VVS', 'VVSS', 'SSS'):
+        return [np.ones((1,) * len(v.fields), dtype=complex)]
     f = su3.F.astype(complex)
     if v.kind == 'VVV':
         return [f]
@@ -250,8 +276,8 @@ def _slot_order(v, child_fields):
     """Map children (and the remaining line) to the vertex tensor's axes.
 
     Returns (axes of the children, axis of the remaining line)."""
-    if v.kind == 'FFV':
-        roles = {v.row: 0, v.col: 1, v.vec: 2}
+    if v.kind in ('FFV', 'FFS'):
+        roles = {v.row: 0, v.col: 1, (v.vec if v.kind == 'FFV' else v.sca): 2}
         ax = [roles[f] for f in child_fields]
         rem = [a for a in (0, 1, 2) if a not in ax]
         return ax, (rem[0] if rem else None)
@@ -310,6 +336,8 @@ class Kinematics:
                         w = D.u_spinor(pi, m, lam) if is_part else D.bar(D.v_spinor(pi, m, lam))
                     else:
                         w = D.bar(D.u_spinor(pi, m, lam)) if is_part else D.v_spinor(pi, m, lam)
+                elif s == 'S':
+                    w = np.ones(self.n, dtype=complex)
                 else:
                     e = D.polvec(pi, m, lam)
                     w = e if state == 'in' else np.conj(e)
@@ -340,6 +368,26 @@ def _vertex_currents(v, child_fields, child_vals, child_moms):
         if v.col in vals:  # column continues: i Vslash (..) psi
             return [1j * np.einsum('nab,nb->na', _vslash_coupled(v, vals[v.vec]), vals[v.col])]
         return [1j * np.einsum('na,nab->nb', vals[v.row], _vslash_coupled(v, vals[v.vec]))]
+    if v.kind == 'FFS':
+        vals = dict(zip(child_fields, child_vals))
+        G = v.gl * D.PL + v.gr * D.PR
+        if v.row in vals and v.col in vals:  # -> scalar
+            return [1j * np.einsum('na,ab,nb->n', vals[v.row], G, vals[v.col])]
+        if v.col in vals:
+            return [1j * vals[v.sca][:, None] * np.einsum('ab,nb->na', G, vals[v.col])]
+        return [1j * vals[v.sca][:, None] * np.einsum('na,ab->nb', vals[v.row], G)]
+    if v.kind in ('VVS', 'VVSS', 'SSS'):
+        vecs = [x for f, x in zip(child_fields, child_vals) if spin(f) == 'V']
+        scas = [x for f, x in zip(child_fields, child_vals) if spin(f) == 'S']
+        c = 1j * v.g
+        for x in scas:
+            c = c * x
+        nvec = sum(1 for f in v.fields if spin(f) == 'V')
+        if len(vecs) == nvec == 2:      # both vectors given -> scalar line (or closed on a scalar)
+            return [c * D.mdot(vecs[0], vecs[1])]
+        if nvec == 2:                   # one vector given -> the other vector, index raised by g^{mu nu}
+            return [c[:, None] * vecs[0]] if np.ndim(c) else [c * vecs[0]]
+        return [c if np.ndim(c) else c * np.ones(child_vals[0].shape[0], dtype=complex)]  # SSS
     if v.kind == 'VVV':
         v1, v2 = child_vals
         k1, k2 = child_moms
@@ -358,6 +406,8 @@ def _propagate(field, K, cur, par):
     m, w = mass_width(field, par)
     den = D.mdot(K, K) - m * m + 1j * m * w
     s = spin(field)
+    if s == 'S':
+        return 1j * cur / den
     if s == 'V':
         if m == 0.0:
             return -1j * cur / den[:, None]
@@ -406,7 +456,9 @@ def root_amplitudes(root, hel, kin, memo=None):
     out = []
     for combo in itertools.product(*lists):
         for cur in _vertex_currents(v, fields, list(combo), moms):
-            if spin(last.field) == 'V':
+            if spin(last.field) == 'S':
+                out.append(cur * wl)
+            elif spin(last.field) == 'V':
                 out.append(D.mdot(cur, wl))
             else:
                 out.append(np.einsum('na,na->n', cur, wl))

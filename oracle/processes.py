@@ -25,6 +25,8 @@ class Process:
 
     def helicities(self, leg):
         name = self.legs[leg][0]
+        if fy.spin(name) == 'S':
+            return (0,)
         if fy.spin(name) == 'V' and fy._F[name][2] is not None:
             return (-1, 0, 1)  # massive vector (never external in the configs)
         return (-1, 1)
@@ -37,8 +39,10 @@ class Process:
 
     def avg_factor(self):
         """1/(2*2) * 1/(n_a n_b) * 1/S_ident   (Eq. 4; A7)."""
-        na, nb = fy.coldim(self.initial[0]), fy.coldim(self.initial[1])
-        return 1.0 / (4.0 * na * nb * self.ident_factor())
+        f = 1.0
+        for i, x in enumerate(self.initial):
+            f /= len(self.helicities(i)) * fy.coldim(x)
+        return f / self.ident_factor()
 
     def diagrams(self, par):
         """Diagram list and the brute-force colour matrix between all (diagram, colour-structure) terms."""
@@ -125,9 +129,18 @@ def config(i):
     if i == 5:
         return Process('udx_epveggg', ['u', 'd~'], ['e+', 've', 'g', 'g', 'g'],
                        ['udw', 'enw', 'uug', 'ddg', 'ggg', 'gggg'])
+    # Higgs-sector processes: every scalar vertex of the library in a small process
+    if i == 6:   # VVS: W* -> W H (Eq. 18a)
+        return Process('udx_epveh', ['u', 'd~'], ['e+', 've', 'h'], ['udw', 'enw', 'wwh'])
+    if i == 7:   # VVS twice, VVSS, SSS: Z* -> Z H H
+        return Process('uux_epemhh', ['u', 'u~'], ['e+', 'e-', 'h', 'h'],
+                       ['uuz', 'eez', 'zzh', 'zzhh', 'hhh'])
+    if i == 8:   # FFS with massive external fermions: q q~ -> t t~ H through g, a, Z (and Z* -> Z H)
+        return Process('uux_ttxh', ['u', 'u~'], ['t', 't~', 'h'],
+                       ['uug', 'ttg', 'uua', 'tta', 'uuz', 'ttz', 'tth', 'zzh'])
     raise ValueError(i)
 
 
 # sqrt(s_hat) [GeV] and number of events of each config (BASELINE.json)
-SQRT_S = {1: 80.0, 2: 500.0, 3: 1000.0, 4: 1500.0, 5: 2000.0}
-N_EVENTS = {1: 1 << 16, 2: 1 << 20, 3: 1 << 22, 4: 1 << 22, 5: 1 << 22}
+SQRT_S = {1: 80.0, 2: 500.0, 3: 1000.0, 4: 1500.0, 5: 2000.0, 6: 500.0, 7: 1000.0, 8: 1000.0}
+N_EVENTS = {1: 1 << 16, 2: 1 << 20, 3: 1 << 22, 4: 1 << 22, 5: 1 << 22, 6: 1 << 20, 7: 1 << 20, 8: 1 << 20}
