@@ -55,9 +55,17 @@ enum hg_process {
   HG_UUX_EPEMG = 2,
   HG_UDX_EPVEGG = 3,
   HG_GG_TTXG_DILEP = 4,
-  HG_UDX_EPVEGGG = 5
+  HG_UDX_EPVEGGG = 5,
+  /* Higgs-sector processes: exercise the FFS, VVS, VVSS and SSS vertices of the library
+   * (Eq. 39, 50-52); no cuts, massive final states from massive RAMBO.
+   *   HG_UDX_EPVEH   u d~ -> e+ ve h      (5 legs)  W* -> W H
+   *   HG_UUX_EPEMHH  u u~ -> e+ e- h h    (6 legs)  Z* -> Z H H: Z Z H twice, Z Z H H, H H H
+   *   HG_GG_TTXH     g g -> t t~ h        (5 legs)  t t H Yukawa on massive external tops (Eq. 20d) */
+  HG_UDX_EPVEH = 6,
+  HG_UUX_EPEMHH = 7,
+  HG_GG_TTXH = 8
 };
-#define HG_N_PROCESS 5
+#define HG_N_PROCESS 8
 #define HG_MAX_EXT 9
 
 /* Standard Model inputs (paper's own: PAPER.md:1075; the configs override them).

@@ -116,9 +116,11 @@ def two_body(P, M2, m1sq, m2sq, uc, uf):
     return boost(p1, P, M, m1sq), boost(p2, P, M, m2sq), pst / (4.0 * math.pi * M)
 
 
-N_FINAL = {1: 2, 2: 3, 3: 4, 5: 5}
-N_DRAWS = {1: 8, 2: 12, 3: 16, 4: 24, 5: 20}
-N_EXT = {1: 4, 2: 5, 3: 6, 4: 9, 5: 7}
+N_FINAL = {1: 2, 2: 3, 3: 4, 5: 5, 6: 3, 7: 4, 8: 3}
+N_DRAWS = {1: 8, 2: 12, 3: 16, 4: 24, 5: 20, 6: 12, 7: 16, 8: 12}
+N_EXT = {1: 4, 2: 5, 3: 6, 4: 9, 5: 7, 6: 5, 7: 6, 8: 5}
+# masses of the final-state legs of the Higgs-sector processes (parameter names; None = massless)
+FINAL_MASSES = {6: (None, None, 'mh'), 7: (None, None, 'mh', 'mh'), 8: ('mt', 'mt', 'mh')}
 
 
 def generate(cfg, seed, first_event, n, rs, par):
@@ -127,6 +129,11 @@ def generate(cfg, seed, first_event, n, rs, par):
     p = np.zeros((n, N_EXT[cfg], 4))
     p[:, 0, 0] = p[:, 1, 0] = p[:, 0, 3] = 0.5 * rs
     p[:, 1, 3] = -0.5 * rs
+    if cfg in FINAL_MASSES:
+        masses = np.stack([np.full(n, par[m] if m else 0.0) for m in FINAL_MASSES[cfg]], axis=1)
+        pf, w = rambo_massive(u, masses, rs)
+        p[:, 2:, :] = pf
+        return p, w
     if cfg != 4:
         pf, w = rambo_massless(u, N_FINAL[cfg], rs)
         p[:, 2:, :] = pf
@@ -152,11 +159,11 @@ def generate(cfg, seed, first_event, n, rs, par):
 def default_cuts(cfg):
     """(pt_jet_min, eta_jet_max, eta_lep_max, dr_jj_min); <= 0 disables.  BASELINE.json configs, scope A11/A12."""
     return {1: (0.0, 0.0, 0.0, 0.0), 2: (20.0, 2.5, 2.5, 0.0), 3: (20.0, 0.0, 0.0, 0.4),
-            4: (20.0, 2.5, 0.0, 0.0), 5: (20.0, 2.5, 0.0, 0.4)}[cfg]
+            4: (20.0, 2.5, 0.0, 0.0), 5: (20.0, 2.5, 0.0, 0.4)}.get(cfg, (0.0, 0.0, 0.0, 0.0))
 
 
-JETS = {1: [], 2: [4], 3: [4, 5], 4: [8], 5: [4, 5, 6]}  # gluon legs
-CHARGED_LEPTONS = {1: [2], 2: [2, 3], 3: [2], 4: [3, 6], 5: [2]}
+JETS = {1: [], 2: [4], 3: [4, 5], 4: [8], 5: [4, 5, 6], 6: [], 7: [], 8: []}  # gluon legs
+CHARGED_LEPTONS = {1: [2], 2: [2, 3], 3: [2], 4: [3, 6], 5: [2], 6: [2], 7: [2, 3], 8: []}
 
 
 def pt(p):

@@ -135,9 +135,8 @@ def config(i):
     if i == 7:   # VVS twice, VVSS, SSS: Z* -> Z H H
         return Process('uux_epemhh', ['u', 'u~'], ['e+', 'e-', 'h', 'h'],
                        ['uuz', 'eez', 'zzh', 'zzhh', 'hhh'])
-    if i == 8:   # FFS with massive external fermions: q q~ -> t t~ H through g, a, Z (and Z* -> Z H)
-        return Process('uux_ttxh', ['u', 'u~'], ['t', 't~', 'h'],
-                       ['uug', 'ttg', 'uua', 'tta', 'uuz', 'ttz', 'tth', 'zzh'])
+    if i == 8:   # FFS with massive external fermions: g g -> t t~ H (Eq. 20d)
+        return Process('gg_ttxh', ['g', 'g'], ['t', 't~', 'h'], ['ttg', 'ggg', 'tth'])
     raise ValueError(i)
 
 

@@ -20,6 +20,9 @@ static const ProcVTable* vtable(int process) {
     case HG_UDX_EPVEGG: return &hg_proc_3;
     case HG_GG_TTXG_DILEP: return &hg_proc_4;
     case HG_UDX_EPVEGGG: return &hg_proc_5;
+    case HG_UDX_EPVEH: return &hg_proc_6;
+    case HG_UUX_EPEMHH: return &hg_proc_7;
+    case HG_GG_TTXH: return &hg_proc_8;
   }
   return nullptr;
 }
@@ -287,6 +290,12 @@ static int check_rs(hg_ctx* ctx, const ProcVTable* vt, int process, double rs, c
     if (!(2.0 * mtmax < rs) || !(mtmin2 > 0) || !(mwmax < sqrt(mtmin2)))
       return fail(ctx, HG_EINVAL, (std::string(who) + ": Breit-Wigner windows not open at this sqrt_s_hat").c_str());
   }
+  // massive final states: the threshold must be open
+  double msum = 0.0;
+  if (process == HG_UDX_EPVEH) msum = ctx->par.mh;
+  if (process == HG_UUX_EPEMHH) msum = 2.0 * ctx->par.mh;
+  if (process == HG_GG_TTXH) msum = 2.0 * ctx->par.mt + ctx->par.mh;
+  if (!(msum < rs)) return fail(ctx, HG_EINVAL, (std::string(who) + ": sqrt_s_hat is below the threshold").c_str());
   (void)vt;
   return HG_OK;
 }

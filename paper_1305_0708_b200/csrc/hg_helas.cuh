@@ -524,4 +524,147 @@ HG_HD Vc<T> jggg_bare(const Vc<T>& v1, const Vc<T>& v2, const Vc<T>& v3, T g2) {
   return w;
 }
 
+// =============================================================================== FFS (Eq. 39)
+// L = psibar (gL PL + gR PR) psi S.  In the chiral basis PL keeps column slots A and pairs them with ROW slots A
+// (psibar = psi^dagger gamma^0 has the conjugate RIGHT part in its slots A), PR pairs slots B with B.
+// iosxxx: amplitude (C.4.1)
+template <int MI, int MO, int G, class T>
+HG_HD cx<T> iosxxx(const Sp<T>& fi, const Sp<T>& fo, cx<T> s, T gL, T gR) {
+  cx<T> r = czero<T>();
+  if ((MI & SLOT_A) && (MO & SLOT_A) && (G & CPL_L)) r = gL * cfma(fo.c[1], fi.c[1], fo.c[0] * fi.c[0]);
+  if ((MI & SLOT_B) && (MO & SLOT_B) && (G & CPL_R)) r = r + gR * cfma(fo.c[3], fi.c[3], fo.c[2] * fi.c[2]);
+  return s * r;
+}
+// hioxxx: off-shell scalar from a fermion pair (C.4.4); d = -1/(q^2 - m^2 + i m Gamma)
+template <int MI, int MO, int G, class T, class D>
+HG_HD cx<T> hioxxx(const Sp<T>& fi, const Sp<T>& fo, T gL, T gR, D d) {
+  cx<T> r = czero<T>();
+  if ((MI & SLOT_A) && (MO & SLOT_A) && (G & CPL_L)) r = gL * cfma(fo.c[1], fi.c[1], fo.c[0] * fi.c[0]);
+  if ((MI & SLOT_B) && (MO & SLOT_B) && (G & CPL_R)) r = r + gR * cfma(fo.c[3], fi.c[3], fo.c[2] * fi.c[2]);
+  return d * r;
+}
+// fsixxx: off-shell flowing-IN fermion  d (qslash + m) (gL PL + gR PR) |fi> S   (C.4.2)
+template <int MI, int G, bool MASSIVE, class T, class D>
+HG_HD Sp<T> fsixxx(const Sp<T>& fi, cx<T> s, T gL, T gR, const Mom<T>& q, T m, D d) {
+  constexpr bool L = (MI & SLOT_A) && (G & CPL_L);  // w_A = gL S fi_A
+  constexpr bool R = (MI & SLOT_B) && (G & CPL_R);  // w_B = gR S fi_B
+  cx<T> wA0 = czero<T>(), wA1 = czero<T>(), wB0 = czero<T>(), wB1 = czero<T>();
+  if (L) {
+    const cx<T> g = gL * s;
+    wA0 = g * fi.c[0];
+    wA1 = g * fi.c[1];
+  }
+  if (R) {
+    const cx<T> g = gR * s;
+    wB0 = g * fi.c[2];
+    wB1 = g * fi.c[3];
+  }
+  Sp<T> f;
+  for (int i = 0; i < 4; ++i) f.c[i] = czero<T>();
+  // (qslash + m) w :  A <- M-(q) w_B + m w_A ,  B <- M+(q) w_A + m w_B
+  if (R || (L && MASSIVE)) {
+    cx<T> y0 = czero<T>(), y1 = czero<T>();
+    if (R) sig_col<-1>(q, wB0, wB1, y0, y1);
+    if (L && MASSIVE) {
+      y0 = y0 + m * wA0;
+      y1 = y1 + m * wA1;
+    }
+    f.c[0] = d * y0;
+    f.c[1] = d * y1;
+  }
+  if (L || (R && MASSIVE)) {
+    cx<T> y0 = czero<T>(), y1 = czero<T>();
+    if (L) sig_col<+1>(q, wA0, wA1, y0, y1);
+    if (R && MASSIVE) {
+      y0 = y0 + m * wB0;
+      y1 = y1 + m * wB1;
+    }
+    f.c[2] = d * y0;
+    f.c[3] = d * y1;
+  }
+  return f;
+}
+// fsoxxx: off-shell flowing-OUT fermion  d <fo| (gL PL + gR PR) S (qslash + m)   (C.4.3)
+template <int MO, int G, bool MASSIVE, class T, class D>
+HG_HD Sp<T> fsoxxx(const Sp<T>& fo, cx<T> s, T gL, T gR, const Mom<T>& q, T m, D d) {
+  constexpr bool L = (MO & SLOT_A) && (G & CPL_L);  // w_A = gL S fo_A
+  constexpr bool R = (MO & SLOT_B) && (G & CPL_R);  // w_B = gR S fo_B
+  cx<T> wA0 = czero<T>(), wA1 = czero<T>(), wB0 = czero<T>(), wB1 = czero<T>();
+  if (L) {
+    const cx<T> g = gL * s;
+    wA0 = g * fo.c[0];
+    wA1 = g * fo.c[1];
+  }
+  if (R) {
+    const cx<T> g = gR * s;
+    wB0 = g * fo.c[2];
+    wB1 = g * fo.c[3];
+  }
+  Sp<T> f;
+  for (int i = 0; i < 4; ++i) f.c[i] = czero<T>();
+  // w (qslash + m) :  A <- w_B M+(q) + m w_A ,  B <- w_A M-(q) + m w_B
+  if (R || (L && MASSIVE)) {
+    cx<T> y0 = czero<T>(), y1 = czero<T>();
+    if (R) sig_row<+1>(q, wB0, wB1, y0, y1);
+    if (L && MASSIVE) {
+      y0 = y0 + m * wA0;
+      y1 = y1 + m * wA1;
+    }
+    f.c[0] = d * y0;
+    f.c[1] = d * y1;
+  }
+  if (L || (R && MASSIVE)) {
+    cx<T> y0 = czero<T>(), y1 = czero<T>();
+    if (L) sig_row<-1>(q, wA0, wA1, y0, y1);
+    if (R && MASSIVE) {
+      y0 = y0 + m * wB0;
+      y1 = y1 + m * wB1;
+    }
+    f.c[2] = d * y0;
+    f.c[3] = d * y1;
+  }
+  return f;
+}
+
+// =============================================================================== VVS, VVSS, SSS (Eq. 50-52)
+// L_VVS = g (V1.V2) S, L_VVSS = g (V1.V2) S3 S4, L_SSS = g S1 S2 S3 (C.7-C.9); g is the
+// coefficient of the Feynman rule (W W H: gW mW, Z Z H: gZ mZ, W W H H: gW^2/2, Z Z H H: gZ^2/2, H H H: -3 mH^2/v).
+template <class T>
+HG_HD cx<T> vvsxxx(const Vc<T>& v1, const Vc<T>& v2, cx<T> s, T g) {
+  return g * (s * vdot(v1, v2));
+}
+// jvsxxx: off-shell vector from a vector and a scalar
+template <bool UNITARY, class T, class D>
+HG_HD Vc<T> jvsxxx(const Vc<T>& v, cx<T> s, T g, const Mom<T>& q, T rm2, D d) {
+  const cx<T> gs = g * s;
+  Vc<T> j;
+  for (int i = 0; i < 4; ++i) j.c[i] = gs * v.c[i];
+  return vprop<UNITARY>(j, q, rm2, d);
+}
+// hvvxxx: off-shell scalar from two vectors; d = -1/(q^2 - m^2 + i m Gamma)
+template <class T, class D>
+HG_HD cx<T> hvvxxx(const Vc<T>& v1, const Vc<T>& v2, T g, D d) {
+  return d * (g * vdot(v1, v2));
+}
+template <class T>
+HG_HD cx<T> vvssxx(const Vc<T>& v1, const Vc<T>& v2, cx<T> s3, cx<T> s4, T g) {
+  return g * (s3 * s4 * vdot(v1, v2));
+}
+template <bool UNITARY, class T, class D>
+HG_HD Vc<T> jvssxx(const Vc<T>& v, cx<T> s3, cx<T> s4, T g, const Mom<T>& q, T rm2, D d) {
+  return jvsxxx<UNITARY>(v, s3 * s4, g, q, rm2, d);
+}
+template <class T, class D>
+HG_HD cx<T> hvvsxx(const Vc<T>& v1, const Vc<T>& v2, cx<T> s, T g, D d) {
+  return d * (g * (s * vdot(v1, v2)));
+}
+template <class T>
+HG_HD cx<T> sssxxx(cx<T> s1, cx<T> s2, cx<T> s3, T g) {
+  return g * (s1 * s2 * s3);
+}
+template <class T, class D>
+HG_HD cx<T> hssxxx(cx<T> s1, cx<T> s2, T g, D d) {
+  return d * (g * (s1 * s2));
+}
+
 }  // namespace hg

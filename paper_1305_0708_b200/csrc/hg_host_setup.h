@@ -32,6 +32,9 @@ inline bool default_cuts(int process, hg_cuts* c) {
     case HG_UDX_EPVEGG: *c = hg_cuts{20.0, 0.0, 0.0, 0.4}; return true;
     case HG_GG_TTXG_DILEP: *c = hg_cuts{20.0, 2.5, 0.0, 0.0}; return true;
     case HG_UDX_EPVEGGG: *c = hg_cuts{20.0, 2.5, 0.0, 0.4}; return true;
+    case HG_UDX_EPVEH:
+    case HG_UUX_EPEMHH:
+    case HG_GG_TTXH: *c = hg_cuts{0.0, 0.0, 0.0, 0.0}; return true;
   }
   return false;
 }
@@ -46,6 +49,7 @@ inline PsConst make_psconst(const hg_params& par, const hg_cuts& cuts, int n_ram
   k.mw = par.mw;
   k.mgw = par.mw * par.gw;
   k.mb2 = par.mb * par.mb;
+  k.mh = par.mh;
   k.tmax_t = par.gt > 0 ? atan(fmin(20.0, par.mt / par.gt)) : 0.0;
   k.tmax_w = par.gw > 0 ? atan(fmin(20.0, par.mw / par.gw)) : 0.0;
   k.pt_jet_min = cuts.pt_jet_min;

@@ -37,6 +37,7 @@ struct PsConst {
   double mt, mgt;  // top: mass, mass*width
   double mw, mgw;  // W
   double mb2;      // m_b^2
+  double mh;       // Higgs mass (final-state mass of the Higgs-sector processes)
   double tmax_t, tmax_w;  // atan(min(20, m/Gamma))  (A.15; reading A14)
   double pt_jet_min, eta_jet_max, eta_lep_max, dr_jj_min;  // cuts, <= 0 disables
 };
@@ -189,6 +190,24 @@ HG_HD double gen_massless(const PsConst& k, uint64_t seed, uint64_t event, uint3
   p[1] = mkmom<double>(h, 0.0, 0.0, -h);
   rambo_massless<NFINAL>(u, k.rs, p + 2);
   return k.vol;
+}
+
+// Final states with massive particles (Higgs-sector processes): massive RAMBO, masses m[i] of the final legs.
+template <int NFINAL>
+HG_HD double gen_massive(const PsConst& k, uint64_t seed, uint64_t event, uint32_t pid, const double (&m)[NFINAL],
+                         Mom<double>* p) {
+  double u[4 * NFINAL];
+  draw_uniforms<4 * NFINAL>(seed, event, pid, u);
+  const double h = 0.5 * k.rs;
+  p[0] = mkmom<double>(h, 0.0, 0.0, h);
+  p[1] = mkmom<double>(h, 0.0, 0.0, -h);
+  double m2[NFINAL], msum = 0.0;
+#pragma unroll
+  for (int i = 0; i < NFINAL; ++i) {
+    m2[i] = m[i] * m[i];
+    msum += m[i];
+  }
+  return k.vol * rambo_massive<NFINAL>(u, m2, msum, k.rs, p + 2);
 }
 
 // config 4: g g -> (t -> b (W+ -> e+ ve)) (t~ -> b~ (W- -> mu- vm~)) g.  Draws: 0-3 s_t, s_t~, s_W+, s_W-;

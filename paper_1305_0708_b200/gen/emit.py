@@ -453,6 +453,34 @@ class CodeGen(Emitter):
             a, b, c3 = kids
             x, y, z = {1: (a, b, c3), 2: (a, c3, b), 3: (b, c3, a)}[nd.struct]
             return 'jgggxx(%s, %s, %s, %s, %s)' % (nm(x), nm(y), nm(z), self._cpl(v.coup[0]), self._d(nd))
+        if v.kind == 'FFS':
+            g = self._gmask(v)
+            gl, gr = self._cpl(v.coup[0]), self._cpl(v.coup[1])
+            if nd.out_slot == 0:    # the column continues
+                col, sca = by_slot[1], by_slot[2]
+                return 'fsixxx<%d, %d, %s>(%s, %s, %s, %s, %s, %s, %s)' % (
+                    mk(col), g, massive, nm(col), nm(sca), gl, gr, self._K(nd.mask), self._mass(p), self._d(nd))
+            if nd.out_slot == 1:    # the row continues
+                row, sca = by_slot[0], by_slot[2]
+                return 'fsoxxx<%d, %d, %s>(%s, %s, %s, %s, %s, %s, %s)' % (
+                    mk(row), g, massive, nm(row), nm(sca), gl, gr, self._Kn(nd.mask), self._mass(p), self._d(nd))
+            row, col = by_slot[0], by_slot[1]
+            return 'hioxxx<%d, %d, %d>(%s, %s, %s, %s, %s)' % (
+                mk(col), mk(row), g, nm(col), nm(row), gl, gr, self._d(nd))
+        if v.kind in ('VVS', 'VVSS'):
+            # slots 0, 1: vectors; 2 (, 3): scalars
+            g = self._cpl(v.coup[0])
+            scas = [nm(by_slot[s_]) for s_ in sorted(by_slot) if s_ >= 2]
+            if nd.out_slot >= 2:    # scalar from the two vectors (and the other scalar)
+                fn = 'hvvxxx' if v.kind == 'VVS' else 'hvvsxx'
+                return '%s(%s)' % (fn, ', '.join([nm(by_slot[0]), nm(by_slot[1])] + scas + [g, self._d(nd)]))
+            vec = by_slot[1 - nd.out_slot]
+            fn = 'jvsxxx' if v.kind == 'VVS' else 'jvssxx'
+            return '%s<%s>(%s)' % (fn, massive, ', '.join([nm(vec)] + scas + [g, self._K(nd.mask), self._rm2(p),
+                                                                             self._d(nd)]))
+        if v.kind == 'SSS':
+            a, b = [by_slot[s_] for s_ in sorted(by_slot)]
+            return 'hssxxx(%s, %s, %s, %s)' % (nm(a), nm(b), self._cpl(v.coup[0]), self._d(nd))
         raise NotImplementedError(v.kind)
 
     def _root_expr(self, rt, vi, hel):
@@ -475,6 +503,14 @@ class CodeGen(Emitter):
             a, b, c3, d4 = [by_slot[s] for s in sorted(by_slot)]
             x, y, z = {1: (a, b, c3), 2: (a, c3, b), 3: (b, c3, a)}[rt.struct]
             return 'ggggxx(%s, %s, %s, %s, %s)' % (nm(x), nm(y), nm(z), nm(d4), self._cpl(v.coup[0]))
+        if v.kind == 'FFS':
+            row, col, sca = by_slot[0], by_slot[1], by_slot[2]
+            return 'iosxxx<%d, %d, %d>(%s, %s, %s, %s, %s)' % (
+                mk(col), mk(row), self._gmask(v), nm(col), nm(row), nm(sca), self._cpl(v.coup[0]),
+                self._cpl(v.coup[1]))
+        if v.kind in ('VVS', 'VVSS', 'SSS'):
+            fn = {'VVS': 'vvsxxx', 'VVSS': 'vvssxx', 'SSS': 'sssxxx'}[v.kind]
+            return '%s(%s)' % (fn, ', '.join([nm(by_slot[s_]) for s_ in sorted(by_slot)] + [self._cpl(v.coup[0])]))
         raise NotImplementedError(v.kind)
 
     def closes_by_current(self):

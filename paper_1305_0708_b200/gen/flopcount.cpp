@@ -12,6 +12,9 @@
 #include "../csrc/generated/hg_proc_3.cuh"
 #include "../csrc/generated/hg_proc_4.cuh"
 #include "../csrc/generated/hg_proc_5.cuh"
+#include "../csrc/generated/hg_proc_6.cuh"
+#include "../csrc/generated/hg_proc_7.cuh"
+#include "../csrc/generated/hg_proc_8.cuh"
 
 using namespace hg;
 
@@ -54,5 +57,8 @@ int main() {
   run<P3>(1000.0);
   run<P4>(1500.0);
   run<P5>(2000.0);
+  run<P6>(500.0);
+  run<P7>(1000.0);
+  run<P8>(1000.0);
   return 0;
 }

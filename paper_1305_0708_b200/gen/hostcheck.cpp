@@ -13,6 +13,9 @@
 #include "../csrc/generated/hg_proc_3.cuh"
 #include "../csrc/generated/hg_proc_4.cuh"
 #include "../csrc/generated/hg_proc_5.cuh"
+#include "../csrc/generated/hg_proc_6.cuh"
+#include "../csrc/generated/hg_proc_7.cuh"
+#include "../csrc/generated/hg_proc_8.cuh"
 
 using namespace hg;
 
@@ -40,6 +43,9 @@ int main() {
       case 3: ok = eval<P3>(c); break;
       case 4: ok = eval<P4>(c); break;
       case 5: ok = eval<P5>(c); break;
+      case 6: ok = eval<P6>(c); break;
+      case 7: ok = eval<P7>(c); break;
+      case 8: ok = eval<P8>(c); break;
     }
     if (!ok) return 1;
   }
