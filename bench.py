@@ -275,7 +275,8 @@ def run_gpu(args):
     e2e_ms = statistics.mean(_events_ms(torch, lambda: ctx.hg_matrix_element_host(cfg, prec, hp, hme), args.steps))
     e2e = {'value': n / (e2e_ms * 1e-3), 'unit': UNIT, 'h2d_bytes_per_step': hp.numel() * el,
            'd2h_bytes_per_step': hme.numel() * el,
-           'what': 'hg_matrix_element_host: pinned host momenta -> H2D -> |Mbar|^2 kernel -> D2H, per step'}
+           'what': 'hg_matrix_element_host: pinned host momenta -> H2D -> |Mbar|^2 kernel -> D2H per step, '
+                   'pipelined in 2^19-event chunks (copy of chunk i+1 overlaps the kernel of chunk i)'}
     del hp, hme
 
     n_pass = acc[3] / world if world > 1 else acc[3]

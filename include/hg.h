@@ -146,8 +146,10 @@ int hg_gen_phase_space(hg_ctx* ctx, int process, int precision, uint64_t seed, u
 int hg_matrix_element(hg_ctx* ctx, int process, int precision, int64_t n, const void* d_p, void* d_me2,
                       void* cuda_stream);
 
-/* Same operation on HOST buffers: copies h_p to a context-owned device staging buffer (grown on demand,
- * released by hg_destroy), runs hg_matrix_element and copies the result back; synchronises the stream. */
+/* Same operation on HOST buffers (pinned memory for full copy speed), pipelined in chunks of 2^19 events through
+ * two context-owned device buffers (grown on demand, released by hg_destroy): the H2D copy of the next chunk runs
+ * on a context-owned stream while the kernel and the D2H copy of the current one run on cuda_stream.
+ * Synchronises cuda_stream before returning. */
 int hg_matrix_element_host(hg_ctx* ctx, int process, int precision, int64_t n, const void* h_p,
                            void* h_me2, void* cuda_stream);
 

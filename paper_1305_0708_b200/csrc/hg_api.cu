@@ -46,6 +46,8 @@ struct hg_ctx {
   size_t stage_bytes = 0;
   void* d_scratch = nullptr;     // phase-space points of one chunk of hg_integrate_step (staged processes)
   size_t scratch_bytes = 0;
+  cudaStream_t copy_stream = nullptr;   // H2D copies of hg_matrix_element_host
+  cudaEvent_t ev_h2d[2] = {nullptr, nullptr}, ev_free[2] = {nullptr, nullptr};
   int profiling = 0;             // hg_set_profiling
   std::vector<cudaEvent_t> ev;   // 3 per chunk
   double t_ps_ms = 0, t_me_ms = 0;
@@ -202,6 +204,11 @@ void hg_destroy(hg_ctx* ctx) {
   if (ctx->d_stage) cudaFree(ctx->d_stage);
   if (ctx->d_scratch) cudaFree(ctx->d_scratch);
   for (cudaEvent_t ev : ctx->ev) cudaEventDestroy(ev);
+  for (int i = 0; i < 2; ++i) {
+    if (ctx->ev_h2d[i]) cudaEventDestroy(ctx->ev_h2d[i]);
+    if (ctx->ev_free[i]) cudaEventDestroy(ctx->ev_free[i]);
+  }
+  if (ctx->copy_stream) cudaStreamDestroy(ctx->copy_stream);
   delete ctx;
 }
 
@@ -337,22 +344,52 @@ int hg_matrix_element_host(hg_ctx* ctx, int process, int precision, int64_t n, c
   if (!vt) return rc;
   if (n == 0) return HG_OK;
   if (!h_p || !h_me2) return fail(ctx, HG_EINVAL, "hg_matrix_element_host: h_p / h_me2 is NULL");
+  // Pipelined in chunks of kHostChunk events over two device buffers: the H2D copy of chunk i+1 (on a context-owned
+  // copy stream) overlaps the kernel and the D2H copy of chunk i (on the caller's stream).  The host array is
+  // [n_ext][4][n], so one chunk is 4 n_ext strided rows: one cudaMemcpy2DAsync.
   const size_t el = precision == HG_F64 ? 8 : 4;
-  const size_t in_bytes = el * 4 * (size_t)vt->info.n_ext * (size_t)n, out_bytes = el * (size_t)n;
-  if (ctx->stage_bytes < in_bytes + out_bytes) {
+  const int rows = 4 * vt->info.n_ext;
+  const int64_t chunk = n < kHostChunk ? n : kHostChunk;
+  const size_t in_bytes = el * rows * (size_t)chunk, out_bytes = el * (size_t)chunk;
+  const size_t buf_bytes = (in_bytes + out_bytes + 255) / 256 * 256;
+  if (ctx->stage_bytes < 2 * buf_bytes) {
     if (ctx->d_stage) cudaFree(ctx->d_stage);
     ctx->d_stage = nullptr;
     ctx->stage_bytes = 0;
-    cudaError_t e = cudaMalloc(&ctx->d_stage, in_bytes + out_bytes);
+    cudaError_t e = cudaMalloc(&ctx->d_stage, 2 * buf_bytes);
     if (e != cudaSuccess) return fail_cuda(ctx, e, "hg_matrix_element_host: cudaMalloc");
-    ctx->stage_bytes = in_bytes + out_bytes;
+    ctx->stage_bytes = 2 * buf_bytes;
+  }
+  cudaError_t e = cudaSuccess;
+  if (!ctx->copy_stream) {
+    e = cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking);
+    for (int i = 0; i < 2 && e == cudaSuccess; ++i) {
+      e = cudaEventCreateWithFlags(&ctx->ev_h2d[i], cudaEventDisableTiming);
+      if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->ev_free[i], cudaEventDisableTiming);
+    }
+    if (e != cudaSuccess) return fail_cuda(ctx, e, "hg_matrix_element_host: stream/event creation");
   }
   cudaStream_t s = (cudaStream_t)cuda_stream;
-  char* d_in = (char*)ctx->d_stage;
-  char* d_out = d_in + in_bytes;
-  cudaError_t e = cudaMemcpyAsync(d_in, h_p, in_bytes, cudaMemcpyHostToDevice, s);
-  if (e == cudaSuccess) e = vt->me(precision, n, d_in, d_out, ctx->coup, s);
-  if (e == cudaSuccess) e = cudaMemcpyAsync(h_me2, d_out, out_bytes, cudaMemcpyDeviceToHost, s);
+  // the copy stream must not start before work already queued on the caller's stream that uses the buffers
+  e = cudaEventRecord(ctx->ev_free[0], s);
+  if (e == cudaSuccess) e = cudaEventRecord(ctx->ev_free[1], s);
+  int i = 0;
+  for (int64_t off = 0; off < n && e == cudaSuccess; off += chunk, ++i) {
+    const int64_t m = n - off < chunk ? n - off : chunk;
+    const int b = i & 1;
+    char* d_in = (char*)ctx->d_stage + (size_t)b * buf_bytes;
+    char* d_out = d_in + in_bytes;
+    e = cudaStreamWaitEvent(ctx->copy_stream, ctx->ev_free[b], 0);   // buffer b no longer read by chunk i-2
+    if (e == cudaSuccess)
+      e = cudaMemcpy2DAsync(d_in, el * (size_t)m, (const char*)h_p + el * (size_t)off, el * (size_t)n,
+                            el * (size_t)m, rows, cudaMemcpyHostToDevice, ctx->copy_stream);
+    if (e == cudaSuccess) e = cudaEventRecord(ctx->ev_h2d[b], ctx->copy_stream);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(s, ctx->ev_h2d[b], 0);
+    if (e == cudaSuccess) e = vt->me(precision, m, d_in, d_out, ctx->coup, s);
+    if (e == cudaSuccess)
+      e = cudaMemcpyAsync((char*)h_me2 + el * (size_t)off, d_out, el * (size_t)m, cudaMemcpyDeviceToHost, s);
+    if (e == cudaSuccess) e = cudaEventRecord(ctx->ev_free[b], s);
+  }
   if (e == cudaSuccess) e = cudaStreamSynchronize(s);
   if (e != cudaSuccess) return fail_cuda(ctx, e, "hg_matrix_element_host");
   return HG_OK;

@@ -15,6 +15,8 @@ constexpr int kIntThreads = 128;
 constexpr int kMaxPartialBlocks = 148 * 16;
 // events per chunk of the two-kernel step of staged processes (the chunk buffer is 233 MB for W + 3 jets, fp64)
 constexpr int64_t kIntChunk = (int64_t)1 << 20;
+// events per chunk of the copy/compute pipeline of hg_matrix_element_host
+constexpr int64_t kHostChunk = (int64_t)1 << 19;
 
 struct ProcVTable {
   hg_process_info_t info;
