@@ -27,10 +27,10 @@ struct SmemStage {
   __device__ __forceinline__ int hi() const { return half + 1; }
   __device__ __forceinline__ T get(int s) const { return ((volatile T*)b)[s * STRIDE]; }
   __device__ __forceinline__ void put(int s, T v) const { b[s * STRIDE] = v; }
-  // Block-wide rendezvous, emitted by the generator every few calls.  Nothing is exchanged: it keeps the warps of
-  // a block within a few hundred instructions of each other, so that they share instruction-cache lines (the
-  // generated code is 5-10x larger than the 32 KB L1.5 instruction cache; without it every warp streams its own
-  // copy of the code from L2, profiles/r01_notes.md section 3).  Every thread of the block must call me2().
+  // Block-wide rendezvous, emitted by the generator at the top of every helicity-loop iteration: the two warps of
+  // a pair share the loop-level slots, so neither may start writing the values of the next iteration while the
+  // other still reads those of the current one.  It also keeps the warps of a block close together in the code
+  // (shared instruction-cache lines).  Every thread of the block must call me2().
   __device__ __forceinline__ void sync() const { __syncthreads(); }
 };
 #endif

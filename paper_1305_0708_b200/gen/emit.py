@@ -186,7 +186,10 @@ class CodeGen(Emitter):
     liveness left to nvcc (small processes)."""
 
     SIZES = {'T': 1, 'cx<T>': 2, 'Mom<T>': 4, 'Vc<T>': 8, 'pol': 5}
-    SYNC_EVERY = 4     # staged mode: block rendezvous after this many calls (instruction-cache sharing)
+    # staged mode: extra block rendezvous after this many calls inside a loop body.  Tuned on B200: 1, 4, 16 and
+    # none gave 13.35 / 12.90 ms (before the merged currents) and 5.50 / 5.38 / 5.34 ms (after) for cfg 5 fp64, so
+    # only the rendezvous at the top of each loop iteration remains (needed by the pair split, hg_stage.cuh).
+    SYNC_EVERY = 1000
 
     def __init__(self, diag, stage=False, kfromp=False):
         super().__init__(diag)
