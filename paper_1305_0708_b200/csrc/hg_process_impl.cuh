@@ -21,8 +21,8 @@ namespace hg {
 // A staged process (P::n_stage > 0) keeps P::n_stage words per EVENT in shared memory, which is what limits the
 // events in flight on an SM (227 KB).  Each event is evaluated by a PAIR of warps (pair split): warps 2g and 2g+1
 // of a block hold the same 32 events, share their staging area, and take one iteration each of the innermost
-// helicity loop (SmemStage::lo/hi), which is ~90 % of the work; the helicity-independent part is computed by both
-// (they write identical values to the same slots).  Two warps per scheduler are what hides the instruction-fetch
+// helicity loop (SmemStage::lo/hi), which is ~85 % of the work; the phases outside it are dealt to the two warps
+// by the generator (SmemStage::own), results meeting in the staging area at the next rendezvous.  Two warps per scheduler are what hides the instruction-fetch
 // stall at every 128-byte line of the 170 KB straight-line code (profiles/r01_notes.md section 3).
 constexpr int kSmemPerSM = 227 * 1024;
 template <class P>

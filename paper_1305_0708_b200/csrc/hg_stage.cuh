@@ -25,6 +25,8 @@ struct SmemStage {
   int half;  // which half of the innermost helicity loop this warp evaluates (pair split, hg_process_impl.cuh)
   __device__ __forceinline__ int lo() const { return half; }
   __device__ __forceinline__ int hi() const { return half + 1; }
+  // does this warp evaluate the part of a shared phase dealt to half h? (emit.py _render_shared)
+  __device__ __forceinline__ bool own(int h) const { return half == h; }
   __device__ __forceinline__ T get(int s) const { return ((volatile T*)b)[s * STRIDE]; }
   __device__ __forceinline__ void put(int s, T v) const { b[s * STRIDE] = v; }
   // Block-wide rendezvous, emitted by the generator at the top of every helicity-loop iteration: the two warps of
@@ -41,6 +43,7 @@ struct HostStage {
   void put(int s, T v) const { b[s] = v; }
   int lo() const { return 0; }
   int hi() const { return 2; }
+  bool own(int) const { return true; }
   void sync() const {}
 };
 

@@ -16,6 +16,7 @@ The paper's temporary-variable recycling is left to nvcc's re
 emitted in SSA form inside the loop scope where they live.
 """
 import itertools
+import re
 from fractions import Fraction
 from math import factorial, gcd
 
@@ -190,6 +191,7 @@ class CodeGen(Emitter):
     # none gave 13.35 / 12.90 ms (before the merged currents) and 5.50 / 5.38 / 5.34 ms (after) for cfg 5 fp64, so
     # only the rendezvous at the top of each loop iteration remains (needed by the pair split, hg_stage.cuh).
     SYNC_EVERY = 1000
+    SPLIT_SHARED = True   # deal the phases outside the innermost loop to the two warps of a pair
 
     def __init__(self, diag, stage=False, kfromp=False):
         super().__init__(diag)
@@ -260,6 +262,7 @@ class CodeGen(Emitter):
         self.max_slots = [0, 0]
         self.need_K = set()       # masks whose summed momentum is needed
         self.need_P = set()       # external legs whose momentum is read inside loops (kfromp)
+        self.dup_names = set()    # cheap depth-0 values evaluated by both warps of a pair
         self.need_d = {}          # (mask, field) -> variable name of the propagator factor
         self.need_rm2 = set()     # mass names whose 1/m^2 is needed
         self.shared = {}          # key -> name of depth-0 values already emitted
@@ -293,14 +296,68 @@ class CodeGen(Emitter):
         out = []
         if self.stage:
             out.append('  constexpr int L = %d;  // first slot of the loop-level values' % self.max_slots[0])
-        out += self._render_items(pre, '  ')
-        out += self._render_items(self.shared_items, '  ')
+        out += self._render_shared(pre + self.shared_items, '  ')
         out.append('  T me = T(0);')
         for var in variants:
             out += self._render_variant(var)
         scale = self.avg_factor() / cden
         out.append('  return me * T(%s);' % _lit(scale))
         self.n_stage = self.max_slots[0] + self.max_slots[1] if self.stage else 0
+        return out
+
+    # rough cost (flops) of an emitted call, used only to balance the two halves of a shared phase
+    _CALL_COST = (('fvixxx', 63), ('fvoxxx', 63), ('fsixxx', 40), ('fsoxxx', 40), ('jioxx', 45), ('jvvxxx', 110),
+                  ('jgggxx', 70), ('vxxxxx', 40), ('ixxxx0', 25), ('oxxxx0', 25), ('crcp', 25), ('hrcp', 15),
+                  ('unit0', 18), ('two_dot0', 8))
+
+    def _render_shared(self, items, ind):
+        """A phase that both warps of a pair would execute (everything outside the innermost helicity loop).  Its
+        items are partitioned into groups that do not read each other's registers (values of other loop depths
+        come through the staging area anyway) and the groups are dealt to the two warps, st.own(0) / st.own(1),
+        balanced by estimated cost.  The rendezvous at the top of the next loop makes all results visible."""
+        if not (self.stage and self.SPLIT_SHARED) or any(it[0] != 'def' for it in items) or len(items) < 2:
+            return self._render_items(items, ind)
+        both = [it for it in items if it[1] in self.dup_names]
+        items = [it for it in items if it[1] not in self.dup_names]
+        index = {it[1]: i for i, it in enumerate(items)}
+        parent = list(range(len(items)))
+
+        def find(i):
+            while parent[i] != i:
+                parent[i] = parent[parent[i]]
+                i = parent[i]
+            return i
+
+        cost = []
+        for i, it in enumerate(items):
+            for tok in set(re.findall(r'[A-Za-z_]\w*', it[2])):
+                j = index.get(tok)
+                if j is not None and j != i:
+                    parent[find(i)] = find(j)
+            c = 4
+            for fn, w in self._CALL_COST:
+                if fn in it[2]:
+                    c = w
+                    break
+            cost.append(c)
+        groups = {}
+        for i in range(len(items)):
+            groups.setdefault(find(i), []).append(i)
+        load = [0, 0]
+        owner = {}
+        for root, members in sorted(groups.items(), key=lambda kv: -sum(cost[i] for i in kv[1])):
+            h = 0 if load[0] <= load[1] else 1
+            load[h] += sum(cost[i] for i in members)
+            for i in members:
+                owner[i] = h
+        out = self._render_items(both, ind)
+        for h in (0, 1):
+            mine = [items[i] for i in range(len(items)) if owner[i] == h]
+            if not mine:
+                continue
+            out.append(ind + 'if (st.own(%d)) {  // estimated %d of %d flops of this phase' % (h, load[h], sum(load)))
+            out += self._render_items(mine, ind + '  ')
+            out.append(ind + '}')
         return out
 
     def _render_items(self, items, ind):
@@ -680,7 +737,7 @@ class CodeGen(Emitter):
             b.append(ind + self._dyn_leaf_decl(lg))
             if d == k:
                 b.append(ind + var['accdecl'])
-            b += self._render_items(levels[d], ind)
+            b += self._render_items(levels[d], ind) if d == k else self._render_shared(levels[d], ind)
         for line in var['tail']:
             b.append(ind + line)
         for d in range(k):
@@ -712,14 +769,16 @@ class CodeGen(Emitter):
         L = []
         raw = lambda t: L.append(('raw', t))
 
-        def define(name, ctype, expr):
+        def define(name, ctype, expr, cheap=False):
             self._reg(name, ctype, 0)
+            if cheap:   # a few adds / one reciprocal: evaluated by both warps of a pair (see _render_shared)
+                self.dup_names.add(name)
             L.append(('def', name, expr, []))
 
         n = self.dg.n
         sgn = {l.index: (1 if l.state == 'in' else -1) for l in self.legs}
         for l in sorted(self.need_P):
-            define('P%d' % l, 'Mom<T>', 'p[%d]' % l)
+            define('P%d' % l, 'Mom<T>', 'p[%d]' % l, cheap=True)
         # momenta of sub-sets (all-incoming: initial +p, final -p)
         have = {}
         for m in sorted(self.need_K, key=lambda m: (_popcount(m), m)):
@@ -737,22 +796,22 @@ class CodeGen(Emitter):
                         pairs.add((ls[a], ls[b2]))
         units = sorted({l for pr in pairs for l in pr if not self.legs[l].particle.mass})
         for l in units:
-            raw('const Mom<T> n%d = unit0(p[%d]);' % (l, l))
+            define('n%d' % l, 'Mom<T>', 'unit0(p[%d])' % l, cheap=True)
         for (a, b2) in sorted(pairs):
             s = '' if sgn[a] * sgn[b2] > 0 else '-'
             if not self.legs[a].particle.mass and not self.legs[b2].particle.mass:
-                raw('const T t%d_%d = %stwo_dot0(n%d, n%d);' % (a, b2, s, a, b2))
+                define('t%d_%d' % (a, b2), 'T', '%stwo_dot0(n%d, n%d)' % (s, a, b2), cheap=True)
             else:
-                raw('const T t%d_%d = %sT(2) * mdot(p[%d], p[%d]);' % (a, b2, s, a, b2))
+                define('t%d_%d' % (a, b2), 'T', '%sT(2) * mdot(p[%d], p[%d])' % (s, a, b2), cheap=True)
         for m, use in sorted(q2.items()):
             ls = list(bits(use))
             terms = ['t%d_%d' % (ls[a], ls[b2]) for a in range(len(ls)) for b2 in range(a + 1, len(ls))]
             for l in ls:
                 if self.legs[l].particle.mass:
                     terms.append('c.%s * c.%s' % (self.legs[l].particle.mass, self.legs[l].particle.mass))
-            raw('const T q2_%d = %s;' % (m, ' + '.join(terms)))
+            define('q2_%d' % m, 'T', ' + '.join(terms), cheap=True)
         for mass in sorted(self.need_rm2):
-            define('rm2_%s' % mass, 'T', 'hrcp(c.%s * c.%s)' % (mass, mass))
+            define('rm2_%s' % mass, 'T', 'hrcp(c.%s * c.%s)' % (mass, mass), cheap=True)
         for (m, mass, width, spin), name in sorted(self.need_d.items()):
             sign = '' if spin == 'V' else '-'
             den = 'q2_%d' % m if not mass else '(q2_%d - c.%s * c.%s)' % (m, mass, mass)
@@ -773,10 +832,10 @@ class CodeGen(Emitter):
         hi = max(bits(m))
         rest = m & ~(1 << hi)
         if rest == 0:
-            define('K%d' % m, 'Mom<T>', '%sp[%d]' % ('' if sgn[hi] > 0 else '-', hi))
+            define('K%d' % m, 'Mom<T>', '%sp[%d]' % ('' if sgn[hi] > 0 else '-', hi), cheap=True)
         else:
             self._emit_K(rest, have, define, sgn)
-            define('K%d' % m, 'Mom<T>', 'K%d %s p[%d]' % (rest, '+' if sgn[hi] > 0 else '-', hi))
+            define('K%d' % m, 'Mom<T>', 'K%d %s p[%d]' % (rest, '+' if sgn[hi] > 0 else '-', hi), cheap=True)
         have[m] = True
 
 
