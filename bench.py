@@ -32,11 +32,12 @@ if ROOT not in sys.path:
 
 METRIC = 'helicity+colour-summed |M|^2 events/s on 1 B200; % of FP64/FP32 peak'
 UNIT = 'events/s'
-SQRT_S = {1: 80.0, 2: 500.0, 3: 1000.0, 4: 1500.0, 5: 2000.0, 6: 500.0, 7: 1000.0, 8: 1000.0}
-N_EVENTS = {1: 1 << 16, 2: 1 << 20, 3: 1 << 22, 4: 1 << 22, 5: 1 << 22, 6: 1 << 20, 7: 1 << 20, 8: 1 << 20}
+SQRT_S = {1: 80.0, 2: 500.0, 3: 1000.0, 4: 1500.0, 5: 2000.0, 6: 500.0, 7: 1000.0, 8: 1000.0, 9: 3000.0}
+N_EVENTS = {1: 1 << 16, 2: 1 << 20, 3: 1 << 22, 4: 1 << 22, 5: 1 << 22, 6: 1 << 20, 7: 1 << 20, 8: 1 << 20, 9: 1 << 20}
 NAMES = {1: 'u d~ -> e+ ve', 2: 'u u~ -> e+ e- g', 3: 'u d~ -> e+ ve g g',
          4: 'g g -> t t~ g -> b e+ ve b~ mu- vm~ g', 5: 'u d~ -> e+ ve g g g',
-         6: 'u d~ -> e+ ve h', 7: 'u u~ -> e+ e- h h', 8: 'g g -> t t~ h'}   # 6-8: Higgs-sector (NEXT-1)
+         6: 'u d~ -> e+ ve h', 7: 'u u~ -> e+ e- h h', 8: 'g g -> t t~ h',   # 6-8: Higgs-sector (NEXT-1)
+         9: 'u d~ -> e+ ve g g g g'}                                          # W + 4 jets (NEXT-4)
 SEED = 13050708
 # nominal non-tensor peaks of B200: 148 SMs x 4 SMSP x 16 lanes x 2 flop x 1.965 GHz for
 # FP64 (one DFMA warp instruction per SMSP every 2 cycles) and twice that for FP32
@@ -97,7 +98,7 @@ class ClockSampler:
 
 
 # ------------------------------------------------------------------------------------------ oracle timing
-ORACLE_SAMPLE = {1: 65536, 2: 8192, 3: 2048, 4: 48, 5: 48, 6: 8192, 7: 4096, 8: 1024}   # events per oracle step (about 1-3 s each)
+ORACLE_SAMPLE = {1: 65536, 2: 8192, 3: 2048, 4: 48, 5: 48, 6: 8192, 7: 4096, 8: 1024, 9: 4}   # events per oracle step (about 1-3 s each)
 
 
 def oracle_step(cfg, first, n):
@@ -304,7 +305,7 @@ def run_gpu(args):
 
     per_config = {}
     if not args.no_table:
-        for c in (1, 2, 3, 4, 5, 6, 7, 8):
+        for c in (1, 2, 3, 4, 5, 6, 7, 8, 9):
             for pr, nm in ((api.HG_F64, 'f64'), (api.HG_F32, 'f32')):
                 per_config['cfg%d_%s' % (c, nm)] = measure_config(torch, api, ctx, c, pr, N_EVENTS[c], 7, peaks)
         per_config['cfg1_f64_4M'] = measure_config(torch, api, ctx, 1, api.HG_F64, 1 << 22, 7, peaks)
@@ -336,7 +337,7 @@ def main():
     ap.add_argument('--gpus', type=int, default=1)
     ap.add_argument('--steps', type=int, default=20)
     ap.add_argument('--warmup', type=int, default=3)
-    ap.add_argument('--config', type=int, default=5, choices=[1, 2, 3, 4, 5, 6, 7, 8])
+    ap.add_argument('--config', type=int, default=5, choices=[1, 2, 3, 4, 5, 6, 7, 8, 9])
     ap.add_argument('--dtype', default='f64', choices=['f64', 'f32'])
     ap.add_argument('--events', type=int, default=0, help='events per GPU per step (default: BASELINE.json size)')
     ap.add_argument('--impl', default='graft', choices=['graft', 'reference'])

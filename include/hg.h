@@ -63,9 +63,12 @@ enum hg_process {
    *   HG_GG_TTXH     g g -> t t~ h        (5 legs)  t t H Yukawa on massive external tops (Eq. 20d) */
   HG_UDX_EPVEH = 6,
   HG_UUX_EPEMHH = 7,
-  HG_GG_TTXH = 8
+  HG_GG_TTXH = 8,
+  /* next size up: u d~ -> e+ ve g g g g, 8 legs, 428 Feynman diagrams / 516
+   * colour-split amplitudes, 24 colour flows, 16 of 256 helicity combinations non-zero; cuts as config 5 */
+  HG_UDX_EPVEGGGG = 9
 };
-#define HG_N_PROCESS 8
+#define HG_N_PROCESS 9
 #define HG_MAX_EXT 9
 
 /* Standard Model inputs (paper's own: PAPER.md:1075; the configs override them).

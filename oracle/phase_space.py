@@ -116,9 +116,9 @@ def two_body(P, M2, m1sq, m2sq, uc, uf):
     return boost(p1, P, M, m1sq), boost(p2, P, M, m2sq), pst / (4.0 * math.pi * M)
 
 
-N_FINAL = {1: 2, 2: 3, 3: 4, 5: 5, 6: 3, 7: 4, 8: 3}
-N_DRAWS = {1: 8, 2: 12, 3: 16, 4: 24, 5: 20, 6: 12, 7: 16, 8: 12}
-N_EXT = {1: 4, 2: 5, 3: 6, 4: 9, 5: 7, 6: 5, 7: 6, 8: 5}
+N_FINAL = {1: 2, 2: 3, 3: 4, 5: 5, 6: 3, 7: 4, 8: 3, 9: 6}
+N_DRAWS = {1: 8, 2: 12, 3: 16, 4: 24, 5: 20, 6: 12, 7: 16, 8: 12, 9: 24}
+N_EXT = {1: 4, 2: 5, 3: 6, 4: 9, 5: 7, 6: 5, 7: 6, 8: 5, 9: 8}
 # masses of the final-state legs of the Higgs-sector processes (parameter names; None = massless)
 FINAL_MASSES = {6: (None, None, 'mh'), 7: (None, None, 'mh', 'mh'), 8: ('mt', 'mt', 'mh')}
 
@@ -159,11 +159,11 @@ def generate(cfg, seed, first_event, n, rs, par):
 def default_cuts(cfg):
     """(pt_jet_min, eta_jet_max, eta_lep_max, dr_jj_min); <= 0 disables.  BASELINE.json configs, scope A11/A12."""
     return {1: (0.0, 0.0, 0.0, 0.0), 2: (20.0, 2.5, 2.5, 0.0), 3: (20.0, 0.0, 0.0, 0.4),
-            4: (20.0, 2.5, 0.0, 0.0), 5: (20.0, 2.5, 0.0, 0.4)}.get(cfg, (0.0, 0.0, 0.0, 0.0))
+            4: (20.0, 2.5, 0.0, 0.0), 5: (20.0, 2.5, 0.0, 0.4), 9: (20.0, 2.5, 0.0, 0.4)}.get(cfg, (0.0, 0.0, 0.0, 0.0))
 
 
-JETS = {1: [], 2: [4], 3: [4, 5], 4: [8], 5: [4, 5, 6], 6: [], 7: [], 8: []}  # gluon legs
-CHARGED_LEPTONS = {1: [2], 2: [2, 3], 3: [2], 4: [3, 6], 5: [2], 6: [2], 7: [2, 3], 8: []}
+JETS = {1: [], 2: [4], 3: [4, 5], 4: [8], 5: [4, 5, 6], 6: [], 7: [], 8: [], 9: [4, 5, 6, 7]}  # gluon legs
+CHARGED_LEPTONS = {1: [2], 2: [2, 3], 3: [2], 4: [3, 6], 5: [2], 6: [2], 7: [2, 3], 8: [], 9: [2]}
 
 
 def pt(p):

@@ -11,7 +11,7 @@ import torch
 
 HG_F64, HG_F32 = 0, 1
 HG_UDX_EPVE, HG_UUX_EPEMG, HG_UDX_EPVEGG, HG_GG_TTXG_DILEP, HG_UDX_EPVEGGG = 1, 2, 3, 4, 5
-PROCESSES = (1, 2, 3, 4, 5)
+PROCESSES = (1, 2, 3, 4, 5, 6, 7, 8, 9)
 HG_OK, HG_EINVAL, HG_ENOPROC, HG_ECUDA, HG_ENOTSET = 0, -1, -2, -3, -4
 
 # symbols include/hg.h declares (checked by tests/test_abi.py)

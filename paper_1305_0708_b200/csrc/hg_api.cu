@@ -23,6 +23,7 @@ static const ProcVTable* vtable(int process) {
     case HG_UDX_EPVEH: return &hg_proc_6;
     case HG_UUX_EPEMHH: return &hg_proc_7;
     case HG_GG_TTXH: return &hg_proc_8;
+    case HG_UDX_EPVEGGGG: return &hg_proc_9;
   }
   return nullptr;
 }

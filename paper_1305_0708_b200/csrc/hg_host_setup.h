@@ -31,7 +31,8 @@ inline bool default_cuts(int process, hg_cuts* c) {
     case HG_UUX_EPEMG: *c = hg_cuts{20.0, 2.5, 2.5, 0.0}; return true;
     case HG_UDX_EPVEGG: *c = hg_cuts{20.0, 0.0, 0.0, 0.4}; return true;
     case HG_GG_TTXG_DILEP: *c = hg_cuts{20.0, 2.5, 0.0, 0.0}; return true;
-    case HG_UDX_EPVEGGG: *c = hg_cuts{20.0, 2.5, 0.0, 0.4}; return true;
+    case HG_UDX_EPVEGGG:
+    case HG_UDX_EPVEGGGG: *c = hg_cuts{20.0, 2.5, 0.0, 0.4}; return true;
     case HG_UDX_EPVEH:
     case HG_UUX_EPEMHH:
     case HG_GG_TTXH: *c = hg_cuts{0.0, 0.0, 0.0, 0.0}; return true;

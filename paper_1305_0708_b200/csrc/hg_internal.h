@@ -39,6 +39,6 @@ struct ProcVTable {
   size_t (*scratch_bytes_per_event)(int prec);
 };
 
-extern const ProcVTable hg_proc_1, hg_proc_2, hg_proc_3, hg_proc_4, hg_proc_5, hg_proc_6, hg_proc_7, hg_proc_8;
+extern const ProcVTable hg_proc_1, hg_proc_2, hg_proc_3, hg_proc_4, hg_proc_5, hg_proc_6, hg_proc_7, hg_proc_8, hg_proc_9;
 
 }  // namespace hg

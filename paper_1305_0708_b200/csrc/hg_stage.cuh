@@ -115,6 +115,14 @@ HG_HD void st_sp(const St& st, int s, const Sp<T>& f) {
     st_cx<T>(st, o + 2, f.c[3]);
   }
 }
+// colour-flow accumulators kept in the staging area (processes with many flows): (X, Y) += k (rb, ib)
+template <class T, class St>
+HG_HD void acc_add(const St& st, int s, T k, cx<T> rb, cx<T> ib) {
+  st.put(s, st.get(s) + k * rb.re);
+  st.put(s + 1, st.get(s + 1) + k * rb.im);
+  st.put(s + 2, st.get(s + 2) + k * ib.re);
+  st.put(s + 3, st.get(s + 3) + k * ib.im);
+}
 // polarisation vector of a massless vector leg, helicity +1: eps^0 = 0 and eps^3 is real, so 5 words.
 // flip != 0 returns the helicity -1 vector -conj(eps) (vflip).
 template <class T, class St>

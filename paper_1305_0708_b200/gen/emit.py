@@ -191,6 +191,7 @@ class CodeGen(Emitter):
     # none gave 13.35 / 12.90 ms (before the merged currents) and 5.50 / 5.38 / 5.34 ms (after) for cfg 5 fp64, so
     # only the rendezvous at the top of each loop iteration remains (needed by the pair split, hg_stage.cuh).
     SYNC_EVERY = 1000
+    ACC_IN_REGS_MAX = 8   # colour-flow accumulators stay in registers up to this many flows
     SPLIT_SHARED = True   # deal the phases outside the innermost loop to the two warps of a pair
 
     def __init__(self, diag, stage=False, kfromp=False):
@@ -657,6 +658,13 @@ class CodeGen(Emitter):
         fidx = {w: i for i, w in enumerate(self.flows)}
         inner = levels[k]
         last = self.dg.last
+        # Many colour flows (W + 4 jets: 24): the 2 nf complex accumulators would take 8 nf registers of fp64, so
+        # they live in the staging area instead, one set per warp of the pair.
+        acc_smem = cbc and self.stage and nf > self.ACC_IN_REGS_MAX
+        if acc_smem:
+            accbase = self.n_slots[1]
+            self.n_slots[1] += 8 * nf
+            self.max_slots[1] = max(self.max_slots[1], self.n_slots[1])
         for rt in roots:
             for ch in rt.children:
                 need(ch)
@@ -668,7 +676,9 @@ class CodeGen(Emitter):
                 lines.append('close_proj(%s, b, rb, ib);' % self._ref('e%d' % last))
                 for w, cf in sorted(rt.colour.terms.items()):
                     f = fidx[w]
-                    if cf == 1:
+                    if acc_smem:
+                        lines.append('acc_add<T>(st, A + %d, T(%d), rb, ib);' % (4 * f, cf))
+                    elif cf == 1:
                         lines.append('X%d = X%d + rb; Y%d = Y%d + ib;' % (f, f, f, f))
                     elif cf == -1:
                         lines.append('X%d = X%d - rb; Y%d = Y%d - ib;' % (f, f, f, f))
@@ -691,8 +701,13 @@ class CodeGen(Emitter):
             tail.append('#pragma unroll')
             tail.append('for (int h%d = 0; h%d < 2; ++h%d) {' % (last, last, last))
             tail.append('  const T sg = h%d ? T(-1) : T(1);' % last)
-            tail.append('  const cx<T> ' + ', '.join('j%d = close_amp(X%d, Y%d, sg)' % (f, f, f) for f in range(nf))
-                        + ';')
+            if acc_smem:
+                tail.append('  const cx<T> ' + ', '.join(
+                    'j%d = close_amp(ld_cx<T>(st, A + %d), ld_cx<T>(st, A + %d), sg)' % (f, 4 * f, 4 * f + 2)
+                    for f in range(nf)) + ';')
+            else:
+                tail.append('  const cx<T> ' + ', '.join('j%d = close_amp(X%d, Y%d, sg)' % (f, f, f)
+                                                         for f in range(nf)) + ';')
         pre = '  ' if cbc else ''
         for f in range(nf):
             terms = []
@@ -703,7 +718,11 @@ class CodeGen(Emitter):
                 terms.append('T(%d) * j%d' % (cval, g))
             tail.append(pre + '{ const cx<T> t = %s; me += j%d.re * t.re + j%d.im * t.im; }' % (
                 ' + '.join(terms), f, f))
-        if cbc:
+        if cbc and acc_smem:
+            tail.append('}')
+            accdecl = ('const int A = L + %d + st.lo() * %d; for (int i = 0; i < %d; ++i) st.put(A + i, T(0));'
+                       % (accbase, 4 * nf, 4 * nf))
+        elif cbc:
             tail.append('}')
             accdecl = 'cx<T> ' + ', '.join('X%d = czero<T>(), Y%d = czero<T>()' % (f, f) for f in range(nf)) + ';'
         else:

@@ -15,6 +15,7 @@
 #include "../csrc/generated/hg_proc_6.cuh"
 #include "../csrc/generated/hg_proc_7.cuh"
 #include "../csrc/generated/hg_proc_8.cuh"
+#include "../csrc/generated/hg_proc_9.cuh"
 
 using namespace hg;
 
@@ -60,5 +61,6 @@ int main() {
   run<P6>(500.0);
   run<P7>(1000.0);
   run<P8>(1000.0);
+  run<P9>(3000.0);
   return 0;
 }

@@ -16,6 +16,7 @@
 #include "../csrc/generated/hg_proc_6.cuh"
 #include "../csrc/generated/hg_proc_7.cuh"
 #include "../csrc/generated/hg_proc_8.cuh"
+#include "../csrc/generated/hg_proc_9.cuh"
 
 using namespace hg;
 
@@ -46,6 +47,7 @@ int main() {
       case 6: ok = eval<P6>(c); break;
       case 7: ok = eval<P7>(c); break;
       case 8: ok = eval<P8>(c); break;
+      case 9: ok = eval<P9>(c); break;
     }
     if (!ok) return 1;
   }

@@ -22,8 +22,8 @@ PAR = osm.default_params()
 SEED = 13050708
 # events per config for the element-by-element comparison: several 128-thread blocks and a ragged tail, sized so
 # that the oracle finishes in seconds (it costs 15 us .. 50 ms per event)
-N_PARITY = {1: 65536, 2: 4099, 3: 1283, 4: 259, 5: 259, 6: 4099, 7: 1283, 8: 515}
-ALL = [1, 2, 3, 4, 5, 6, 7, 8]     # 6-8: Higgs-sector processes
+N_PARITY = {1: 65536, 2: 4099, 3: 1283, 4: 259, 5: 259, 6: 4099, 7: 1283, 8: 515, 9: 67}
+ALL = [1, 2, 3, 4, 5, 6, 7, 8, 9]  # 6-8: Higgs-sector processes (NEXT-1); 9: W + 4 jets (NEXT-4)
 MASSIVE_PS = (4, 6, 7, 8)        # phase space with a Newton solve (massive RAMBO)
 
 
@@ -283,7 +283,7 @@ def test_edge_cases_and_errors(ctx, api):
     ref = opr.me2(opr.config(5), p.cpu().numpy().transpose(2, 0, 1), PAR)
     assert abs(me.item() - ref[0]) <= 1e-11 * ref[0]
     with pytest.raises(HgError) as ei:
-        ctx.hg_integrate_step(9, api.HG_F64, 1, 0, 10, 1000.0)
+        ctx.hg_integrate_step(77, api.HG_F64, 1, 0, 10, 1000.0)
     assert ei.value.code == api.HG_ENOPROC
     with pytest.raises(HgError) as ei:
         ctx.hg_integrate_step(3, 7, 1, 0, 10, 1000.0)
