@@ -162,13 +162,15 @@ int hg_matrix_element_host(hg_ctx* ctx, int process, int precision, int64_t n, c
 int hg_accumulate(hg_ctx* ctx, int precision, int64_t n, const void* d_me2, const void* d_wps,
                   const uint8_t* d_pass, double sqrt_s_hat, double acc[4], void* cuda_stream);
 
-/* Steps a1-a10 in one call.  Configs 1-3: fused in one kernel -- each thread draws its event, builds momenta,
- * applies the cuts, evaluates |Mbar|^2 only if it passes, forms w in pb and the block reduces (sum w, sum w^2,
- * n_pass); nothing per-event touches HBM.  Configs 4-5 (matrix elements staged in shared memory at 8 warps per
- * SM): per chunk of 2^20 events a phase-space kernel writes the points to a context-owned buffer (grown on
- * demand, freed by hg_destroy), a compaction kernel lists the passing events in order, and a third kernel
- * evaluates |Mbar|^2 of exactly those and reduces; same results, fixed summation order.  Synchronises the stream; acc (HOST, overwritten) = (sum w, sum w^2, n,
- * n_pass).  sigma = acc[0]/acc[2]. */
+/* Steps a1-a10 in one call.
+ * Configs 1, 3 and process 6: fused in one kernel -- each thread draws its event, builds momenta, applies the
+ * cuts, evaluates |Mbar|^2 only if it passes, forms w in pb and the block reduces (sum w, sum w^2, n_pass);
+ * nothing per-event touches HBM.
+ * Configs 2, 4, 5 and processes 7-9: per chunk of 2^20 events a phase-space kernel (at full occupancy) writes the
+ * points to a context-owned buffer (grown on demand, freed by hg_destroy), a compaction kernel lists the passing
+ * events in order, and a third kernel evaluates |Mbar|^2 of exactly those (staged matrix elements at 8-12 warps per
+ * SM) and reduces.  Same results as the fused form, fixed summation order.
+ * Synchronises the stream; acc (HOST, overwritten) = (sum w, sum w^2, n, n_pass).  sigma = acc[0]/acc[2]. */
 int hg_integrate_step(hg_ctx* ctx, int process, int precision, uint64_t seed, uint64_t first_event,
                       int64_t n, double sqrt_s_hat, double acc[4], void* cuda_stream);
 

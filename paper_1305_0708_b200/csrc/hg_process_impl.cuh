@@ -280,7 +280,7 @@ struct Launch {
                                  cudaEvent_t* ev, cudaStream_t s) {
     constexpr int TH = int_thr<T>();
     constexpr size_t smem = stage_bytes<P, T, TH>();
-    if constexpr (P::n_stage == 0) {
+    if constexpr (!P::split_step) {
       if (ev) cudaEventRecord(ev[0], s);
       integrate_kernel<P, T, TH><<<nblocks, TH, smem, s>>>(k, seed, first, n, c, wscale, d_partials);
       if (ev) cudaEventRecord(ev[2], s);
@@ -314,7 +314,7 @@ struct Launch {
     return ((size_t)chunk * P::n_ext * 4 * sizeof(T) + 255) / 256 * 256;
   }
   static size_t scratch_bytes_per_event(int prec) {
-    if (P::n_stage == 0) return 0;
+    if (!P::split_step) return 0;
     return (size_t)P::n_ext * 4 * (prec == HG_F64 ? 8 : 4) + 8 + 4 + 1;  // momenta, weight, index, pass flag
   }
   static cudaError_t integrate(int prec, int64_t n, const PsConst& k, uint64_t seed, uint64_t first,
@@ -329,7 +329,7 @@ struct Launch {
   static cudaError_t int_blocks_t(int* out) {
     constexpr int TH = int_thr<T>();
     constexpr size_t smem = stage_bytes<P, T, TH>();
-    if constexpr (P::n_stage == 0) {
+    if constexpr (!P::split_step) {
       return cudaOccupancyMaxActiveBlocksPerMultiprocessor(out, integrate_kernel<P, T, TH>, TH, smem);
     } else {
       cudaError_t err = allow_smem(me_acc_kernel<P, T, TH>, smem);
