@@ -701,7 +701,11 @@ class CodeGen(Emitter):
             tail.append('#pragma unroll')
             tail.append('for (int h%d = 0; h%d < 2; ++h%d) {' % (last, last, last))
             tail.append('  const T sg = h%d ? T(-1) : T(1);' % last)
-            if not acc_smem:
+            if acc_smem:
+                tail.append('  const cx<T> ' + ', '.join(
+                    'j%d = close_amp(ld_cx<T>(st, A + %d), ld_cx<T>(st, A + %d), sg)' % (f, 4 * f, 4 * f + 2)
+                    for f in range(nf)) + ';')
+            else:
                 tail.append('  const cx<T> ' + ', '.join('j%d = close_amp(X%d, Y%d, sg)' % (f, f, f)
                                                          for f in range(nf)) + ';')
         pre = '  ' if cbc else ''
@@ -711,19 +715,9 @@ class CodeGen(Emitter):
                 cval = cmat[f][g] * (1 if g == f else 2)
                 if cval == 0:
                     continue
-                if acc_smem:    # partial amplitudes are formed from the staged accumulators where they are used
-                    terms.append('T(%d) * close_amp(ld_cx<T>(st, A + %d), ld_cx<T>(st, A + %d), sg)' % (
-                        cval, 4 * g, 4 * g + 2))
-                else:
-                    terms.append('T(%d) * j%d' % (cval, g))
-            if acc_smem:
-                tail.append(pre + '{ const cx<T> t = %s;' % ' + '.join(terms))
-                tail.append(pre + '  const cx<T> j = close_amp(ld_cx<T>(st, A + %d), ld_cx<T>(st, A + %d), sg);' % (
-                    4 * f, 4 * f + 2))
-                tail.append(pre + '  me += j.re * t.re + j.im * t.im; }')
-            else:
-                tail.append(pre + '{ const cx<T> t = %s; me += j%d.re * t.re + j%d.im * t.im; }' % (
-                    ' + '.join(terms), f, f))
+                terms.append('T(%d) * j%d' % (cval, g))
+            tail.append(pre + '{ const cx<T> t = %s; me += j%d.re * t.re + j%d.im * t.im; }' % (
+                ' + '.join(terms), f, f))
         if cbc and acc_smem:
             tail.append('}')
             accdecl = ('const int A = L + %d + st.lo() * %d; for (int i = 0; i < %d; ++i) st.put(A + i, T(0));'
