@@ -152,3 +152,50 @@ def test_helicity_zero_counts():
         tot = sum(per.values())
         nz = [h for h, v in per.items() if np.max(v / tot) > 1e-20]
         assert len(per) == ntot and len(nz) == nnz, (cfg, len(per), len(nz))
+
+
+# ----------------------------------------------------------------------------- NEXT-1 / NEXT-4 processes
+def test_ward_identity_gg_ttxh():
+    """g g -> t t~ H (process 8): both gluons, external tops on shell; Gamma_t = 0 because a fixed width in the
+    internal top propagators breaks the identity at O(Gamma_t/m_t) (same as config 4, reading A13)."""
+    par = dict(PAR, gt=0.0)
+    proc = P.config(8)
+    p = ps.generate(8, 77, 0, 4, P.SQRT_S[8], par)[0]
+    for leg in (0, 1):
+        assert _ward_residual(proc, p, par, leg) < 1e-22
+
+
+@pytest.mark.parametrize("cfg", [6, 7, 8])
+def test_lorentz_invariance_higgs_processes(cfg):
+    par = dict(PAR, gt=0.0) if cfg == 8 else PAR
+    proc = P.config(cfg)
+    p = ps.generate(cfg, 77, 0, 12, P.SQRT_S[cfg], par)[0]
+    m = P.me2(proc, p, par)
+    m2 = P.me2(proc, inputs.lorentz(p), par)
+    assert np.max(np.abs(m2 / m - 1)) < 1e-10
+
+
+def test_bose_symmetry_zhh():
+    """u u~ -> e+ e- H H: exchanging the two Higgs momenta leaves |M|^2 unchanged."""
+    proc = P.config(7)
+    p = ps.generate(7, 77, 0, 12, P.SQRT_S[7], PAR)[0]
+    q = p.copy()
+    q[:, [4, 5]] = p[:, [5, 4]]
+    assert np.max(np.abs(P.me2(proc, q, PAR) / P.me2(proc, p, PAR) - 1)) < 1e-12
+
+
+def test_w4j_counts_and_ward_identity():
+    """W + 4 jets (process 9): 428 diagrams / 516 colour-split terms (24 flows on the device side), and the Ward
+    identity of one gluon on one event (every relative sign and colour factor of the 516 terms enters it)."""
+    proc = P.config(9)
+    roots, cm, _ = proc.diagrams(PAR)
+    assert len(roots) == 428 and cm.shape == (516, 516)
+    p = ps.generate(9, 77, 0, 1, P.SQRT_S[9], PAR)[0]
+
+    def hook(kin):      # eps(g, leg 7) -> p/E for both helicities; colour summed with the 516 x 516 matrix
+        for lam in (-1, 1):
+            kin.wf[(7, lam)] = p[:, 7, :].astype(complex) / p[:, 7, 0:1]
+
+    # a^dagger C a with 516 terms that cancel among themselves: rounding leaves ~1e-15 of the physical value; a wrong
+    # sign or colour factor anywhere leaves O(1e-3 .. 1)
+    assert np.max(P.me2(proc, p, PAR, wf_hook=hook) / P.me2(proc, p, PAR)) < 1e-12
