@@ -30,7 +30,8 @@ constexpr int kSplit = P::n_stage > 0 ? 2 : 1;
 template <class P, class T>
 constexpr int stage_threads(int want) {
   if (P::n_stage == 0) return want;
-  const int groups = kSmemPerSM / (P::n_stage * (int)sizeof(T) * 32);  // 32-event groups that fit on an SM
+  // 32-event groups that fit on an SM, leaving 3 KB for the kernels' static shared memory
+  const int groups = (kSmemPerSM - 3072) / (P::n_stage * (int)sizeof(T) * 32);
   // 2, 4 or 6 pairs = 4, 8 or 12 warps: a multiple of the 4 schedulers (6 and 10 warps measured slower than 4 and 8)
   const int g = groups >= 6 ? 6 : (groups >= 4 ? 4 : (groups >= 2 ? 2 : 1));
   return 64 * g;
