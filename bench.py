@@ -39,6 +39,9 @@ NAMES = {1: 'u d~ -> e+ ve', 2: 'u u~ -> e+ e- g', 3: 'u d~ -> e+ ve g g',
          6: 'u d~ -> e+ ve h', 7: 'u u~ -> e+ e- h h', 8: 'g g -> t t~ h',   # 6-8: Higgs-sector (NEXT-1)
          9: 'u d~ -> e+ ve g g g g'}                                          # W + 4 jets (NEXT-4)
 SEED = 13050708
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel, from the ncu --set full captures
+# summarised in profiles/ (r01_ncu_full_me_acc_cfg5_f64.txt: 247.76 MB + 4.13 MB; ..._cfg4_f64.txt; ..._w4j_f64.txt)
+TRAFFIC = {'cfg5_f64': 251886592, 'cfg4_f64': 319316480, 'cfg9_f64': 117643264}
 # nominal non-tensor peaks of B200: 148 SMs x 4 SMSP x 16 lanes x 2 flop x 1.965 GHz for
 # FP64 (one DFMA warp instruction per SMSP every 2 cycles) and twice that for FP32
 PEAK_NOMINAL_TFLOPS = {'f64': 148 * 64 * 2 * 1.965e9 / 1e12, 'f32': 148 * 128 * 2 * 1.965e9 / 1e12}
@@ -286,10 +289,7 @@ def run_gpu(args):
     me_ms_step = me_ms / args.steps                      # all launches of the dominant kernel in one step
     flops_kernel = info['flops_f64'] * n_pass + (0.0 if staged else info['flops_ps'] * n)
     achieved = flops_kernel / (me_ms_step * 1e-3) / 1e12
-    traffic = None
-    tpath = os.path.join(ROOT, 'profiles', 'roofline_traffic.json')
-    if os.path.exists(tpath):
-        traffic = json.load(open(tpath)).get('cfg%d_%s' % (cfg, pname))
+    traffic = TRAFFIC.get('cfg%d_%s' % (cfg, pname))
     tname = 'double' if pname == 'f64' else 'float'
     roofline = {'bound': 'alu',
                 'kernel': ('me_acc_kernel<P%d,%s>' if staged else 'integrate_kernel<P%d,%s>') % (cfg, tname),
