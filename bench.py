@@ -40,8 +40,8 @@ NAMES = {1: 'u d~ -> e+ ve', 2: 'u u~ -> e+ e- g', 3: 'u d~ -> e+ ve g g',
          9: 'u d~ -> e+ ve g g g g'}                                          # W + 4 jets (NEXT-4)
 SEED = 13050708
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel, from the ncu --set full captures
-# summarised in profiles/ (r01_ncu_full_me_acc_cfg5_f64.txt: 247.76 MB + 4.13 MB; ..._cfg4_f64.txt; ..._w4j_f64.txt)
-TRAFFIC = {'cfg5_f64': 251886592, 'cfg4_f64': 319316480, 'cfg9_f64': 117643264}
+# summarised in profiles/ (r01_ncu_full_me_acc_cfg5_f64.txt: 247.76 MB + 4.13 MB; r01_ncu_full_me_acc_cfg4_f64.txt: 315.32 MB + 4.00 MB)
+TRAFFIC = {'cfg5_f64': 251886592, 'cfg4_f64': 319316480}
 # nominal non-tensor peaks of B200: 148 SMs x 4 SMSP x 16 lanes x 2 flop x 1.965 GHz for
 # FP64 (one DFMA warp instruction per SMSP every 2 cycles) and twice that for FP32
 PEAK_NOMINAL_TFLOPS = {'f64': 148 * 64 * 2 * 1.965e9 / 1e12, 'f32': 148 * 128 * 2 * 1.965e9 / 1e12}
