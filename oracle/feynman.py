@@ -152,6 +152,7 @@ def build_vertices(par, names):
 class Leaf:
     def __init__(self, leg, field):
         self.leg, self.field, self.legs = leg, field, (leg,)
+        self.sig = 'L%d' % leg
 
 
 class Node:
@@ -160,76 +161,85 @@ class Node:
     def __init__(self, vertex, children, field):
         self.vertex, self.children, self.field = vertex, children, field
         self.legs = tuple(sorted(l for ch in children for l in ch.legs))
+        # structural name of the subtree: equal subtrees of different diagrams have equal names (used only to
+        # avoid evaluating the same sub-diagram twice, see kin_terms)
+        self.sig = '(%s|%s:%s)' % (field, ','.join(vertex.fields), ' '.join(ch.sig for ch in children))
 
 
-def _remaining(vertex, fields):
-    """Fields of `vertex` left over after removing `fields` (multiset), or None if not contained."""
-    rest = list(vertex.fields)
-    for f in fields:
-        if f in rest:
+def _grow(shape, leg):
+    """All shapes obtained from `shape` by attaching `leg`.  A shape is what hangs below a line: an external leg
+    (an int) or a vertex (a tuple of the shapes below its 2 or 3 other lines).  The new leg goes on the line above
+    `shape` (a new three-point vertex), on a three-point vertex (making it a four-point vertex), or anywhere
+    further down."""
+    yield (shape, leg)
+    if isinstance(shape, tuple):
+        if len(shape) == 2:
+            yield shape + (leg,)
+        for i, sub in enumerate(shape):
+            for g in _grow(sub, leg):
+                yield shape[:i] + (g,) + shape[i + 1:]
+
+
+def topologies(n):
+    """All tree topologies with n labelled external legs and vertices of degree 3 and 4, hung from leg n-1, by the
+    textbook recursion: the topologies with one more leg are obtained by attaching the new leg to every line
+    (external lines included) and to every three-point vertex.  Removing that leg again undoes exactly one such
+    step, so every topology is produced once: 1, 4, 25, 220, 2485, 34300 for n = 3 .. 8."""
+    shapes = [(0, 1)]
+    for leg in range(2, n - 1):
+        shapes = [g for s in shapes for g in _grow(s, leg)]
+    return shapes
+
+
+def _vertex_tables(vertices):
+    """closed[sorted fields] = vertex;  open_[sorted fields but one] = [(vertex, the missing field), ...]."""
+    closed, open_ = {}, {}
+    for v in vertices:
+        closed[tuple(sorted(v.fields))] = v
+        for f in set(v.fields):
+            rest = list(v.fields)
             rest.remove(f)
-        else:
-            return None
-    return rest
-
-
-def _partitions(items, nparts):
-    """Unordered partitions of the tuple `items` into `nparts` non-empty groups."""
-    items = tuple(items)
-    if nparts == 1:
-        yield (items,)
-        return
-    first, rest = items[0], items[1:]
-    for r in range(0, len(rest) - nparts + 2):
-        for extra in itertools.combinations(rest, r):
-            g1 = (first,) + extra
-            left = tuple(x for x in rest if x not in extra)
-            for sub in _partitions(left, nparts - 1):
-                yield (g1,) + sub
+            open_.setdefault(tuple(sorted(rest)), []).append((v, f))
+    return closed, open_
 
 
 def enumerate_diagrams(ext_fields, vertices):
-    """All tree diagrams for external all-incoming fields `ext_fields`.
+    """All tree diagrams for external all-incoming fields `ext_fields` (Eq. 6: the sum runs over
+    "all Feynman diagrams of the subprocess").
 
-    Returns a list of root Nodes whose children include Leaf(n-1) as the LAST child.
-    """
+    Two steps: (1) every topology of `topologies(n)`; (2) every way of putting fields of the model on its internal
+    lines such that each point is a vertex of the model: going through the topology from the outside inwards, the
+    fields arriving at a point fix, through the vertex table, the fields the point can send on; the point that
+    carries the last leg must close.
+
+    Returns a list of root Nodes whose children include Leaf(n-1) as the LAST child."""
     n = len(ext_fields)
-    memo = {}
+    closed, open_ = _vertex_tables(vertices)
 
-    def subtrees(legs):
-        if legs in memo:
-            return memo[legs]
-        res = []
-        if len(legs) == 1:
-            res.append(Leaf(legs[0], ext_fields[legs[0]]))
-        else:
-            for npart in (2, 3):
-                if len(legs) < npart:
-                    continue
-                for groups in _partitions(legs, npart):
-                    for combo in itertools.product(*[subtrees(g) for g in groups]):
-                        fs = [t.field for t in combo]
-                        for v in vertices:
-                            if len(v.fields) != npart + 1:
-                                continue
-                            rest = _remaining(v, fs)
-                            if rest is not None:
-                                res.append(Node(v, list(combo), anti(rest[0])))
-        memo[legs] = res
-        return res
+    def dressed(shape):
+        if not isinstance(shape, tuple):
+            return [Leaf(shape, ext_fields[shape])]
+        parts = []
+        for sub in shape:
+            d = dressed(sub)
+            if not d:
+                return []
+            parts.append(d)
+        found = []
+        for kids in itertools.product(*parts):
+            for v, missing in open_.get(tuple(sorted(t.field for t in kids)), ()):
+                found.append(Node(v, list(kids), anti(missing)))
+        return found
 
     last = Leaf(n - 1, ext_fields[n - 1])
     roots = []
-    others = tuple(range(n - 1))
-    for npart in (2, 3):
-        if len(others) < npart:
-            continue
-        for groups in _partitions(others, npart):
-            for combo in itertools.product(*[subtrees(g) for g in groups]):
-                fs = [t.field for t in combo] + [last.field]
-                for v in vertices:
-                    if len(v.fields) == npart + 1 and _remaining(v, fs) == []:
-                        roots.append(Node(v, list(combo) + [last], None))
+    for top in topologies(n):
+        parts = [dressed(sub) for sub in top]
+        if all(parts):
+            for kids in itertools.product(*parts):
+                v = closed.get(tuple(sorted([t.field for t in kids] + [last.field])))
+                if v is not None:
+                    roots.append(Node(v, list(kids) + [last], None))
     return roots
 
 
@@ -425,7 +435,7 @@ def kin_terms(tree, hel, kin, memo=None):
         return [kin.wf[(tree.leg, hel[tree.leg])]]
     key = None
     if memo is not None:
-        key = (id(tree), tuple(hel[l] for l in tree.legs))
+        key = (tree.sig, tuple(hel[l] for l in tree.legs))
         if key in memo:
             return memo[key]
     v = tree.vertex

@@ -10,6 +10,9 @@ import numpy as np
 from . import feynman as fy
 
 
+_DIAGRAM_CACHE = {}   # diagram lists are built once per (process, parameters) and session
+
+
 class Process:
     def __init__(self, name, initial, final, vertex_names):
         self.name = name
@@ -17,7 +20,6 @@ class Process:
         self.legs = [(x, 'in') for x in initial] + [(x, 'out') for x in final]
         self.ext_fields = [x for x in initial] + [fy.anti(x) for x in final]
         self.vertex_names = list(vertex_names)
-        self._cache = {}
 
     @property
     def n_ext(self):
@@ -46,8 +48,8 @@ class Process:
 
     def diagrams(self, par):
         """Diagram list and the brute-force colour matrix between all (diagram, colour-structure) terms."""
-        key = tuple(sorted(par.items()))
-        if key not in self._cache:
+        key = (self.name, tuple(self.legs), tuple(self.vertex_names), tuple(sorted(par.items())))
+        if key not in _DIAGRAM_CACHE:
             verts = fy.build_vertices(par, self.vertex_names)
             roots = fy.enumerate_diagrams(self.ext_fields, verts)
             cols = []
@@ -55,8 +57,8 @@ class Process:
                 cols += [c.reshape(-1) for c in fy.root_colour(r)]
             cmat = np.array(cols)  # [n_terms, prod(colour dims)]
             cm = cmat @ np.conj(cmat.T)  # CM[l,l'] = sum_ext c_l conj(c_l')
-            self._cache[key] = (roots, cm, cmat)
-        return self._cache[key]
+            _DIAGRAM_CACHE[key] = (roots, cm, cmat)
+        return _DIAGRAM_CACHE[key]
 
 
 def amplitudes(proc, p, par, hel, memo=None, kin=None):
