@@ -21,7 +21,9 @@ spinors and polarisation vectors, SU(3) identities, closed-form 2->2 |M|^2
 (u d~ -> e+ ve, q q~ -> a a, u u~ -> e+ e-, q q~ -> t t~, g g -> t t~, q q~ -> g g,
 g g -> g g), Ward identities, Lorentz invariance, Bose symmetry, soft-gluon limit,
 diagram counts, Philox known-answer vectors, RAMBO volumes and energy moments,
-Breit-Wigner integral, analytic sigma(u d~ -> e+ ve).
+Breit-Wigner integral, analytic sigma(u d~ -> e+ ve), the nested phase-space volume of config 4, the position
+of the propagator pole (sign of the width term), the exact factorisation of config 4 on the resonance poles
+into undecayed g g -> t t~ g times the textbook top-decay matrix elements.
 
 Parity status: configs 1 and 2 are pinned to closed forms.  Configs 3, 4, 5 have no printed
 number in the paper: they are pinned by Ward identity + Lorentz/Bose invariance + the

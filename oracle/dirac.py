@@ -7,7 +7,8 @@ matrices is used here on purpose (the device library uses the chiral one, SURVEY
 helicity-summed |M|^2 does not depend on the choice.
 
 All functions are vectorised over a leading event axis: p has shape [N,4] = (E,px,py,pz),
-metric (+,-,-,-).
+metric (+,-,-,-).  The arithmetic runs in the dtype of p: float64 normally, numpy.longdouble (x87 80-bit,
+eps = 1.1e-19) when the caller passes extended-precision momenta (oracle.processes.me2_extended).
 """
 import numpy as np
 
@@ -32,7 +33,7 @@ def mdot(a, b):
 def slash(v):
     """v_mu gamma^mu for v = v^mu of shape [N,4] -> [N,4,4]."""
     vl = v * METRIC  # lower the index
-    return np.einsum('nm,mab->nab', vl.astype(complex), GAM)
+    return np.einsum('nm,mab->nab', vl + 0j, GAM)
 
 
 def _chi(p, lam):
@@ -97,7 +98,7 @@ def polvec(p, m, lam):
     sphi = np.where(ptsafe, py / np.where(ptsafe, pt, 1.0), 0.0)
     zero = np.zeros_like(E)
     if lam == 0:
-        return np.stack([pabs / m, E / m * st * cphi, E / m * st * sphi, E / m * ct], axis=1).astype(complex)
+        return np.stack([pabs / m, E / m * st * cphi, E / m * st * sphi, E / m * ct], axis=1) + 0j
     e1 = np.stack([zero, ct * cphi, ct * sphi, -st], axis=1)  # theta^ direction
     e2 = np.stack([zero, -sphi, cphi, zero], axis=1)  # phi^ direction
-    return (-lam * e1 - 1j * e2) / np.sqrt(2.0)
+    return (-lam * e1 - 1j * e2) / np.sqrt(E.dtype.type(2))

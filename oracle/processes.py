@@ -77,7 +77,9 @@ def me2(proc, p, par, per_helicity=False, batch=2048, wf_hook=None):
 
     wf_hook(kin), if given, may replace external wavefunctions in kin.wf before evaluation (used by the
     Ward-identity pins: polarisation vector -> momentum)."""
-    p = np.asarray(p, dtype=float)
+    p = np.asarray(p)
+    if p.dtype != np.longdouble:
+        p = p.astype(float)
     N = p.shape[0]
     if N > batch:
         parts = [me2(proc, p[i:i + batch], par, per_helicity, batch, wf_hook) for i in range(0, N, batch)]
@@ -87,7 +89,7 @@ def me2(proc, p, par, per_helicity=False, batch=2048, wf_hook=None):
     if wf_hook is not None:
         wf_hook(kin)
     memo = {}
-    total = np.zeros(N)
+    total = np.zeros(N, dtype=p.dtype)
     per = {}
     for hel in itertools.product(*[proc.helicities(i) for i in range(proc.n_ext)]):
         a = amplitudes(proc, p, par, hel, memo, kin)  # [n_terms, N]
@@ -98,6 +100,25 @@ def me2(proc, p, par, per_helicity=False, batch=2048, wf_hook=None):
     if per_helicity:
         return per
     return total * proc.avg_factor()
+
+
+def me2_extended(proc, p, par, on_shell=True, batch=512):
+    """|Mbar|^2 with the same plain formulas evaluated in extended precision (numpy.longdouble: the x87 80-bit
+    format, eps = 1.1e-19, about 3.3 decimal digits more than fp64).  The arbiter when the fp64 oracle and the
+    kernel differ by more than the tolerance (reading A21).
+
+    on_shell=True (reading A21): an external leg is on its mass shell by definition (Eq. 29-33, PAPER.md:412-447,
+    are functions of an on-shell momentum), so its energy is a function of its 3-momentum, E = sqrt(|p|^2 + m^2),
+    taken here in extended precision; the fp64 energy that came with the input is that value rounded.  With
+    on_shell=False the energies are used as given (then p^2 - m^2 = O(eps E^2) enters every invariant that
+    contains the leg).  Returns float64."""
+    p = np.asarray(p).astype(np.longdouble)
+    if on_shell:
+        p = p.copy()
+        for i, (name, _) in enumerate(proc.legs):
+            m, _w = fy.mass_width(name, par)
+            p[:, i, 0] = np.sqrt(p[:, i, 1] ** 2 + p[:, i, 2] ** 2 + p[:, i, 3] ** 2 + np.longdouble(m) ** 2)
+    return me2(proc, p, par, batch=batch).astype(np.float64)
 
 
 def me2_explicit_colour(proc, p, par):

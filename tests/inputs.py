@@ -55,3 +55,35 @@ def lorentz(p, beta=(0.3, -0.2, 0.4), angles=(0.7, 1.1)):
     R = np.array([[1, 0, 0], [0, np.cos(a), -np.sin(a)], [0, np.sin(a), np.cos(a)]]) @ \
         np.array([[np.cos(b), -np.sin(b), 0], [np.sin(b), np.cos(b), 0], [0, 0, 1]])
     return np.concatenate([E2[..., None], v2 @ R.T], -1)
+
+
+def boost_from_rest(pr, P):
+    """pr[..., 4] given in the rest frame of a particle with momentum P[4] (mass from P) -> the frame of P (pure boost)."""
+    P = np.asarray(P, dtype=float)
+    M = np.sqrt(mdot(P, P))
+    e = (P[0] * pr[..., 0] + pr[..., 1:] @ P[1:]) / M
+    fac = (e + pr[..., 0]) / (P[0] + M)
+    return np.concatenate([e[..., None], pr[..., 1:] + fac[..., None] * P[1:]], -1)
+
+
+def decay(P, m1, m2, nhat):
+    """Two-body decay of momentum P into masses (m1, m2); particle 1 leaves along the unit vector nhat in the rest
+    frame of P.  Returns (p1, p2) in the frame of P."""
+    P = np.asarray(P, dtype=float)
+    M = np.sqrt(mdot(P, P))
+    k = np.sqrt(max((M * M - m1 * m1 - m2 * m2) ** 2 - 4 * m1 * m1 * m2 * m2, 0.0)) / (2 * M)
+    nhat = np.asarray(nhat, dtype=float)
+    p1 = np.concatenate([[np.sqrt(k * k + m1 * m1)], k * nhat])
+    p2 = np.concatenate([[np.sqrt(k * k + m2 * m2)], -k * nhat])
+    return boost_from_rest(p1, P), boost_from_rest(p2, P)
+
+
+def tetrahedron(rot=0.0):
+    """Four unit vectors forming a spherical 2-design (sums of polynomials of degree <= 2 over them equal the sphere
+    average), rotated about the z axis by `rot` and tilted so that no vector is along an axis."""
+    v = np.array([[1, 1, 1], [1, -1, -1], [-1, 1, -1], [-1, -1, 1]], dtype=float) / np.sqrt(3.0)
+    c, s = np.cos(rot), np.sin(rot)
+    Rz = np.array([[c, -s, 0], [s, c, 0], [0, 0, 1]])
+    a = 0.4
+    Rx = np.array([[1, 0, 0], [0, np.cos(a), -np.sin(a)], [0, np.sin(a), np.cos(a)]])
+    return v @ (Rz @ Rx).T

@@ -1,0 +1,101 @@
+"""Pins of the oracle's treatment of unstable particles (widths, decay chains):  the position of the propagator
+pole (sign of +i m Gamma) and the exact factorisation of the decayed amplitude at
+the resonance poles (config 4 against undecayed g g -> t t~ g, SURVEY.md 8c 'cfg4 decays')."""
+import itertools
+import math
+
+import numpy as np
+import pytest
+
+from oracle import feynman as fy
+from oracle import processes as opr
+from oracle import sm
+import inputs
+
+PAR = sm.default_params()
+
+
+@pytest.mark.parametrize('field', ['h', 'z', 'w+', 't', 't~'])
+def test_propagator_pole_is_in_the_lower_half_plane(field):
+    """A state of mass m and width Gamma evolves as exp(-i m t - Gamma t / 2): as a function of complex energy (at
+    rest) its propagator has the pole of the positive-energy state at E = sqrt(m^2 - i m Gamma) ~ m - i Gamma/2,
+    BELOW the real axis.  This fixes the sign of the width term in 1/(q^2 - m^2 + i m Gamma), which no helicity-
+    summed |M|^2 pin sees (|D|^2 and the gamma/Z interference are even in Gamma).  With the other sign the pole of
+    _propagate moves to m + i Gamma/2 and both assertions fail."""
+    m, w = fy.mass_width(field, PAR)
+    assert m > 0 and w > 0
+    pole = np.sqrt(complex(m * m, -m * w))
+    assert pole.imag < 0 and abs(pole.imag + w / 2) < 1e-3 * w
+
+    def size(E):
+        K = np.array([[E, 0, 0, 0]], dtype=complex)
+        cur = np.ones(1, dtype=complex) if fy.spin(field) == 'S' else np.ones((1, 4), dtype=complex)
+        return float(np.abs(fy._propagate(field, K, cur, PAR)).max())
+
+    on_axis = size(pole.real)                      # a distance Gamma/2 from the pole
+    near = size(pole + 1e-3 * w)                   # 500 times closer
+    mirrored = size(np.conj(pole) + 1e-3 * w)      # the same point reflected above the axis: twice as far
+    assert near > 100 * on_axis          # the pole is there ...
+    assert mirrored < on_axis            # ... and not at the mirror point
+
+
+def _event(n_t, n_wp, n_tb, n_wm, rs=1500.0):
+    """g g -> t t~ g with on-shell tops, then t -> b W+ (W+ along -n_t... b along n_t in the t frame), W+ -> e+ ve
+    (e+ along n_wp in the W frame), same for t~; every resonance exactly on its pole."""
+    mt, mw = PAR['mt'], PAR['mw']
+    tot = np.array([rs, 0.0, 0.0, 0.0])
+    g_dir = np.array([0.3, -0.5, 0.4])
+    g_dir /= np.linalg.norm(g_dir)
+    eg = 210.0
+    mtt = math.sqrt(rs * rs - 2 * rs * eg)
+    g, tt = decay(tot, 0.0, mtt, g_dir)
+    d = np.array([0.6, 0.2, -0.7])
+    d /= np.linalg.norm(d)
+    t, tb = decay(tt, mt, mt, d)
+    b, wp = decay(t, 0.0, mw, n_t)
+    ep, ve = decay(wp, 0.0, 0.0, n_wp)
+    bb, wm = decay(tb, 0.0, mw, n_tb)
+    mu, vm = decay(wm, 0.0, 0.0, n_wm)
+    pa = np.array([rs / 2, 0, 0, rs / 2])
+    pb = np.array([rs / 2, 0, 0, -rs / 2])
+    full = np.array([pa, pb, b, ep, ve, bb, mu, vm, g])
+    prod = np.array([pa, pb, t, tb, g])
+    return full, prod
+
+
+decay = inputs.decay
+
+
+def test_cfg4_factorises_on_the_poles():
+    """With s_t = s_t~ = m_t^2 and s_W+- = m_W^2 exactly, every resonant propagator numerator is the spin sum of
+    on-shell wavefunctions, so the config-4 amplitude is  sum_spins M_prod * M_dec(t) * M_dec(t~) / (i m_t G_t)^2.
+    Averaged over the decay directions the spin correlations drop out (rotational invariance in the top rest frame):
+
+        < |Mbar(g g -> b e+ ve b~ mu- vm~ g)|^2 >  =  |Mbar(g g -> t t~ g)|^2 * prod_{t, t~} [ 1/2 <sum|M_dec|^2> / (m_t G_t)^2 ]
+
+    with the textbook  sum_spins |M(t -> b e+ ve)|^2 = 4 g_W^4 (p_t.p_e+)(p_b.p_ve) / (m_W G_W)^2  on the W pole.
+    The averages are exact sums over spherical 2-designs (the decay matrix is quadratic in the lepton momentum), so
+    the identity holds to rounding, not to O(Gamma/m): it pins the relative signs and factors of the 16 decayed
+    diagrams, the fermion and W propagators with widths, and the t b W / l nu W vertices against the undecayed
+    process (itself pinned by the g g -> t t~ closed form, Ward identity and soft limit)."""
+    mt, gt, mw, gw = PAR['mt'], PAR['gt'], PAR['mw'], PAR['gw']
+    gW = sm.couplings(PAR)['gw']
+    d1, d2 = inputs.tetrahedron(0.3), inputs.tetrahedron(1.1)
+    fulls, decs = [], []
+    for a, b, c, d in itertools.product(range(4), repeat=4):
+        full, prod = _event(d1[a], d2[b], d2[c], d1[d])
+        fulls.append(full)
+        pt_, ptb = prod[2], prod[3]
+        dec_t = 4 * gW ** 4 * inputs.mdot(pt_, full[3]) * inputs.mdot(full[2], full[4]) / (mw * gw) ** 2
+        dec_tb = 4 * gW ** 4 * inputs.mdot(ptb, full[6]) * inputs.mdot(full[5], full[7]) / (mw * gw) ** 2
+        decs.append((dec_t, dec_tb))
+    fulls = np.array(fulls)
+    decs = np.array(decs)
+    lhs = opr.me2(opr.config(4), fulls, PAR).mean()
+    undecayed = opr.Process('gg_ttxg', ['g', 'g'], ['t', 't~', 'g'], ['ttg', 'ggg', 'gggg'])
+    prod_me = opr.me2(undecayed, prod[None], PAR)[0]
+    rhs = prod_me * (0.5 * decs[:, 0].mean() / (mt * gt) ** 2) * (0.5 * decs[:, 1].mean() / (mt * gt) ** 2)
+    assert abs(lhs / rhs - 1) < 1e-9, (lhs, rhs)
+    # the directions matter event by event (spin correlations are there): the identity is not trivially true
+    per_event = opr.me2(opr.config(4), fulls[:8], PAR) / (prod_me * 0.25 * decs[:8, 0] * decs[:8, 1] / (mt * gt) ** 4)
+    assert np.abs(per_event - 1).max() > 0.05
