@@ -104,27 +104,44 @@ class ClockSampler:
 ORACLE_SAMPLE = {1: 65536, 2: 8192, 3: 2048, 4: 48, 5: 48, 6: 8192, 7: 4096, 8: 1024, 9: 4}   # events per oracle step (about 1-3 s each)
 
 
-def oracle_step(cfg, first, n):
-    """One pass of the hot path in the oracle: Philox -> momenta -> cuts -> |Mbar|^2 -> weights -> sums."""
+def oracle_step(cfg, first, n, all_cores):
+    """One pass of the hot path in the oracle: Philox -> momenta -> cuts -> |Mbar|^2 -> weights -> sums; on one
+    thread, or cut into slices over the host cores (oracle/parallel.py: the same functions per slice)."""
     from oracle import integrate as oint
+    from oracle import parallel as opar
     from oracle import sm as osm
-    w, ok = oint.weights(cfg, SEED, first, n, SQRT_S[cfg], osm.default_params())
+    if all_cores:
+        w, ok = opar.weights(cfg, SEED, first, n, SQRT_S[cfg], osm.default_params(),
+                             slice_events=max(1, n // opar.n_workers()))
+    else:
+        w, ok = oint.weights(cfg, SEED, first, n, SQRT_S[cfg], osm.default_params())
     return oint.accumulate(w, ok)
 
 
-def time_oracle(cfg, steps, warmup, n=None):
-    n = n or ORACLE_SAMPLE[cfg]
+def time_oracle(cfg, steps, warmup, n=None, all_cores=True):
+    """The oracle as it stands on the host: events/s on all cores (worker processes) and on one thread."""
+    from oracle import parallel as opar
+    cores = opar.n_workers() if all_cores else 1
+    n1 = n or ORACLE_SAMPLE[cfg]
+    n = n1 * (cores if all_cores else 1)
     for i in range(warmup):
-        oracle_step(cfg, i * n, n)
-    c0, t0 = time.process_time(), time.perf_counter()
+        oracle_step(cfg, i * n, n, all_cores)
+    t0 = time.perf_counter()
     for i in range(steps):
-        oracle_step(cfg, (warmup + i) * n, n)
+        oracle_step(cfg, (warmup + i) * n, n, all_cores)
     wall = time.perf_counter() - t0
-    cpu = time.process_time() - c0
-    cores = max(1, int(round(cpu / wall)))
+    # one thread, one step of the per-core sample
+    os.environ.setdefault('OMP_NUM_THREADS', '1')
+    t1 = time.perf_counter()
+    oracle_step(cfg, 0, n1, False)
+    wall1 = time.perf_counter() - t1
+    opar.close()
     return {'value': steps * n / wall, 'unit': UNIT, 'cores': cores, 'kind': 'oracle',
+            'value_1_process': n1 / wall1,
             'sample': '%d steps of %d events of the same Philox stream (numpy fp64 oracle, all 2^n_ext helicities, '
-                      'brute-force colour); %d host cores present' % (steps, n, os.cpu_count() or 1)}, wall / steps
+                      'brute-force colour) cut into slices over %d worker processes; value_1_process = one step of %d '
+                      'events in this process; %d host cores present' % (steps, n, cores, n1, os.cpu_count() or 1)}, \
+        wall / steps
 
 
 def run_reference(args):
@@ -137,7 +154,7 @@ def run_reference(args):
             'steps': args.steps, 'warmup': args.warmup, 'ms_per_step': sec * 1e3, 'higher_is_better': True,
             'scaling': 'weak', 'vs_baseline': None, 'dtype': 'f64', 'data': 'synthetic',
             'config': {'workload': workload_name(cfg, N_EVENTS[cfg]),
-                       'sample_per_step': ORACLE_SAMPLE[cfg]},
+                       'sample_per_step': ORACLE_SAMPLE[cfg] * base['cores']},
             'cpu_baseline': base,
             'e2e': {'value': base['value'], 'unit': UNIT, 'h2d_bytes_per_step': 0, 'd2h_bytes_per_step': 0},
             'gpu_launches': 0}
@@ -312,7 +329,8 @@ def run_gpu(args):
         per_config['cfg1_f32_4M'] = measure_config(torch, api, ctx, 1, api.HG_F32, 1 << 22, 7, peaks)
 
     cpu_base, _ = time_oracle(cfg, 4, 1)
-    s, ds = api.sigma(acc)
+    s = acc[0] / acc[2]
+    ds = (max(acc[1] / acc[2] - s * s, 0.0) / max(acc[2] - 1.0, 1.0)) ** 0.5
     line = {'metric': METRIC, 'value': value, 'unit': UNIT, 'n_gpus': world, 'steps': args.steps,
             'warmup': max(args.warmup, 3), 'ms_per_step': ms_per_step, 'higher_is_better': True, 'scaling': 'weak',
             'vs_baseline': None, 'dtype': pname, 'data': 'synthetic',

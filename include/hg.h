@@ -18,7 +18,7 @@
  *     unless stated otherwise;
  *   - every call returns 0 on success or a negative hg_status; the message of the last failure of a
  *     context is available from hg_last_error().  Nothing throws across the ABI.  Arguments are validated
- *     before any launch (NULL pointers, n < 0, unknown process/precision, parameters not set).  n == 0 is
+ *     before any launch (NULL or misaligned pointers, n < 0, unknown process/precision, parameters not set).  n == 0 is
  *     a successful no-op.
  *   - results depend only on (params, cuts, process, precision, seed, first_event, n, sqrt_s_hat): event
  *     k always uses Philox counter k (reading SURVEY.md 8c-A15), so batches can be split or sharded.
@@ -110,8 +110,9 @@ typedef struct {
   double flops_ps;    /* same for phase-space generation + cuts (hg_gen_phase_space) */
 } hg_process_info_t;
 
-/* Create / destroy a context bound to one CUDA device.  hg_create selects the device for the calling
- * thread (cudaSetDevice).  Returns HG_ECUDA if the device cannot be used. */
+/* Create / destroy a context bound to one CUDA device.  Every call on the context runs on that device whatever the
+ * calling thread's current device is, and leaves the caller's current device as it found it; d_ pointers and the
+ * stream passed to a call must belong to the context's device.  Returns HG_ECUDA if the device cannot be used. */
 int hg_create(hg_ctx** out, int cuda_device);
 void hg_destroy(hg_ctx* ctx);
 
@@ -174,16 +175,24 @@ int hg_accumulate(hg_ctx* ctx, int precision, int64_t n, const void* d_me2, cons
 int hg_integrate_step(hg_ctx* ctx, int process, int precision, uint64_t seed, uint64_t first_event,
                       int64_t n, double sqrt_s_hat, double acc[4], void* cuda_stream);
 
-/* Measurement helpers for bench.py.  hg_set_profiling(ctx, 1) makes hg_integrate_step record CUDA events on the
- * launching stream around its kernels; hg_last_step_info then returns, for the last hg_integrate_step of the
- * context, out[0] = milliseconds spent in phase-space kernels (0 when the step is one fused kernel), out[1] =
- * milliseconds in the kernel(s) that evaluate the matrix element, out[2] = number of kernels launched. */
-int hg_set_profiling(hg_ctx* ctx, int on);
-int hg_last_step_info(const hg_ctx* ctx, double out[3]);
-
-/* Measured-peak helper for the roofline: runs a register-resident FMA chain on every SM
- * and returns the achieved FLOP/s for the given precision in *flops_per_s.  Synchronises. */
-int hg_measure_fma_peak(hg_ctx* ctx, int precision, double* flops_per_s, void* cuda_stream);
+/* Adaptive sampling grid of the integration (role of the BASES grid: "a grid-optimisation step followed by an
+ * integration step"; the algorithm is the published VEGAS one, reading A22).
+ * Every uniform draw d of an event (n_draws of hg_process_info) has a grid of n_bins bins with edges
+ * 0 = g[d][0] < ... < g[d][n_bins] = 1; the draw picks a bin uniformly and a point inside it, the event weight carries
+ * the Jacobian prod_d n_bins (g[d][i+1] - g[d][i]).
+ *
+ * hg_set_grid: until reset, hg_gen_phase_space and hg_integrate_step of THE PROCESS THE GRID WAS MADE FOR sample
+ * through d_grid ([n_draws][n_bins + 1] doubles, DEVICE memory owned by the caller, read at every call; 2 <= n_bins <=
+ * HG_GRID_MAX_BINS).  If d_hist is not NULL ([n_draws][n_bins] doubles, device, caller-owned, caller-zeroed) every
+ * hg_integrate_step ADDS the sum of w^2 of the passing events per (draw, bin) to it: the grid-optimisation step.
+ * Summation order is fixed (no atomics): same inputs, same histogram.  d_grid == NULL returns to flat sampling.
+ *
+ * hg_grid_refine (host only; h_ pointers are host memory): one VEGAS refinement of every variable's edges from the
+ * accumulated histogram -- smoothing over neighbouring bins, compression ((1 - s)/ln(1/s))^alpha, re-binning to equal
+ * content; a variable whose histogram is empty or not finite keeps its edges.  h_grid is updated in place. */
+#define HG_GRID_MAX_BINS 64
+int hg_set_grid(hg_ctx* ctx, const double* d_grid, int n_bins, double* d_hist);
+int hg_grid_refine(int n_dim, int n_bins, const double* h_hist, double alpha, double* h_grid);
 
 #ifdef __cplusplus
 }

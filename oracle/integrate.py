@@ -12,14 +12,17 @@ from . import processes as pr
 from . import sm
 
 
-def weights(cfg, seed, first_event, n, rs, par, cuts=None, batch=1024, skip_failed=True):
-    """Per-event weights [n] in pb and pass flags, for events first_event.. of config cfg."""
+def weights(cfg, seed, first_event, n, rs, par, cuts=None, batch=1024, skip_failed=True, grid=None, bins_out=None):
+    """Per-event weights [n] in pb and pass flags, for events first_event.. of config cfg.  grid: adaptive grid of
+    oracle.vegas (None = flat); bins_out [n, n_draws] receives the bin of every draw."""
     proc = pr.config(cfg)
     w = np.zeros(n)
     ok_all = np.zeros(n, dtype=bool)
     for i in range(0, n, batch):
         m = min(batch, n - i)
-        p, wps = ps.generate(cfg, seed, first_event + i, m, rs, par)
+        p, wps, bins = ps.generate(cfg, seed, first_event + i, m, rs, par, grid=grid, with_bins=True)
+        if bins_out is not None and bins is not None:
+            bins_out[i:i + m] = bins
         ok = ps.passes(cfg, p, cuts)
         ok_all[i:i + m] = ok
         idx = np.nonzero(ok)[0] if skip_failed else np.arange(m)

@@ -123,9 +123,24 @@ N_EXT = {1: 4, 2: 5, 3: 6, 4: 9, 5: 7, 6: 5, 7: 6, 8: 5, 9: 8}
 FINAL_MASSES = {6: (None, None, 'mh'), 7: (None, None, 'mh', 'mh'), 8: ('mt', 'mt', 'mh')}
 
 
-def generate(cfg, seed, first_event, n, rs, par):
-    """Momenta [n, n_ext, 4] (leg order of oracle.processes.config) and phase-space weight [n]."""
+def generate(cfg, seed, first_event, n, rs, par, grid=None, with_bins=False):
+    """Momenta [n, n_ext, 4] (leg order of oracle.processes.config) and phase-space weight [n].
+
+    grid [n_draws, NB + 1] (oracle.vegas): the Philox uniforms are mapped through the adaptive grid before they are
+    used and the weight carries the Jacobian; with_bins=True also returns the bin of every draw [n, n_draws]."""
     u = philox.uniforms(seed, first_event, n, N_DRAWS[cfg], cfg)
+    if grid is None:
+        p, w = from_uniforms(cfg, u, rs, par)
+        return (p, w, None) if with_bins else (p, w)
+    from . import vegas
+    x, jac, bins = vegas.apply_grid(np.asarray(grid, dtype=float), u)
+    p, w = from_uniforms(cfg, x, rs, par)
+    return (p, w * jac, bins) if with_bins else (p, w * jac)
+
+
+def from_uniforms(cfg, u, rs, par):
+    """Steps a2-a3 for given numbers u [n, n_draws] in (0, 1)."""
+    n = u.shape[0]
     p = np.zeros((n, N_EXT[cfg], 4))
     p[:, 0, 0] = p[:, 1, 0] = p[:, 0, 3] = 0.5 * rs
     p[:, 1, 3] = -0.5 * rs

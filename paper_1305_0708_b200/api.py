@@ -17,7 +17,10 @@ HG_OK, HG_EINVAL, HG_ENOPROC, HG_ECUDA, HG_ENOTSET = 0, -1, -2, -3, -4
 # symbols include/hg.h declares (checked by tests/test_abi.py)
 SYMBOLS = ('hg_create', 'hg_destroy', 'hg_last_error', 'hg_default_params', 'hg_default_cuts', 'hg_process_info',
            'hg_set_params', 'hg_gen_phase_space', 'hg_matrix_element', 'hg_matrix_element_host', 'hg_accumulate',
-           'hg_integrate_step', 'hg_set_profiling', 'hg_last_step_info', 'hg_measure_fma_peak')
+           'hg_integrate_step', 'hg_set_grid', 'hg_grid_refine')
+HG_GRID_MAX_BINS = 64
+# measurement helpers of include/hg_bench.h (bench.py only)
+BENCH_SYMBOLS = ('hg_set_profiling', 'hg_last_step_info', 'hg_measure_fma_peak')
 
 
 class hg_params(C.Structure):
@@ -73,6 +76,8 @@ def load():
     L.hg_matrix_element_host.argtypes = [vp, i32, i32, i64, vp, vp, vp]
     L.hg_accumulate.argtypes = [vp, i32, i64, vp, vp, vp, dbl, C.POINTER(dbl), vp]
     L.hg_integrate_step.argtypes = [vp, i32, i32, u64, u64, i64, dbl, C.POINTER(dbl), vp]
+    L.hg_set_grid.argtypes = [vp, vp, i32, vp]
+    L.hg_grid_refine.argtypes = [i32, i32, vp, dbl, vp]
     L.hg_measure_fma_peak.argtypes = [vp, i32, C.POINTER(dbl), vp]
     L.hg_set_profiling.argtypes = [vp, i32]
     L.hg_last_step_info.argtypes = [vp, C.POINTER(dbl)]
@@ -100,6 +105,18 @@ def hg_process_info(process):
     if rc != HG_OK:
         raise HgError(rc, 'unknown process id')
     return {n: getattr(info, n) for n, _ in hg_process_info_t._fields_}
+
+
+def hg_grid_refine(hist, alpha, grid):
+    """One refinement of the grid [n_dim, n_bins + 1] (host float64 tensor, updated in place) from hist [n_dim, n_bins]."""
+    n_dim, nb1 = grid.shape
+    for t, shape in ((grid, (n_dim, nb1)), (hist, (n_dim, nb1 - 1))):
+        if t.device.type != 'cpu' or t.dtype != torch.float64 or not t.is_contiguous() or tuple(t.shape) != shape:
+            raise ValueError('grid / hist must be contiguous host float64 tensors [n_dim, n_bins + 1] / [n_dim, n_bins]')
+    rc = load().hg_grid_refine(n_dim, nb1 - 1, C.c_void_p(hist.data_ptr()), float(alpha), C.c_void_p(grid.data_ptr()))
+    if rc != HG_OK:
+        raise HgError(rc, 'hg_grid_refine: bad argument')
+    return grid
 
 
 def _dtype(precision):
@@ -193,6 +210,8 @@ class Context:
             raise ValueError('p must be a contiguous host %s tensor' % dt)
         if me2 is None:
             me2 = torch.empty((n,), dtype=dt).pin_memory()
+        if me2.device.type != 'cpu' or me2.dtype != dt or not me2.is_contiguous() or me2.numel() != n:
+            raise ValueError('me2 must be a contiguous host %s tensor with %d elements' % (dt, n))
         self._check(self._L.hg_matrix_element_host(self._h, process, precision, n, _ptr(p), _ptr(me2),
                                                    _stream(stream)))
         return me2
@@ -215,6 +234,20 @@ class Context:
                                               _stream(stream)))
         return tuple(acc)
 
+    def hg_set_grid(self, grid, hist=None):
+        """grid: CUDA float64 tensor [n_draws, n_bins + 1] (kept alive by the context wrapper) or None for flat
+        sampling; hist: CUDA float64 tensor [n_draws, n_bins] that hg_integrate_step adds sum w^2 per bin to."""
+        if grid is None:
+            self._grid = self._hist = None
+            self._check(self._L.hg_set_grid(self._h, None, 0, None))
+            return
+        n_dim, nb1 = grid.shape
+        self._check_tensor(grid, HG_F64, n_dim * nb1, 'grid', torch.float64)
+        if hist is not None:
+            self._check_tensor(hist, HG_F64, n_dim * (nb1 - 1), 'hist', torch.float64)
+        self._grid, self._hist = grid, hist
+        self._check(self._L.hg_set_grid(self._h, _ptr(grid), nb1 - 1, _ptr(hist)))
+
     def hg_set_profiling(self, on):
         self._check(self._L.hg_set_profiling(self._h, 1 if on else 0))
 
@@ -229,10 +262,3 @@ class Context:
         self._check(self._L.hg_measure_fma_peak(self._h, precision, C.byref(out), _stream(stream)))
         return out.value
 
-
-def sigma(acc):
-    """sigma = sum w / N and its Monte-Carlo standard error from (sum w, sum w^2, N, N_pass)."""
-    sw, sw2, n, _ = acc
-    s = sw / n
-    var = max(sw2 / n - s * s, 0.0) / max(n - 1.0, 1.0)
-    return s, var ** 0.5

@@ -22,22 +22,94 @@ def sources():
     return [os.path.join(CSRC, 'hg_api.cu')] + sorted(glob.glob(os.path.join(CSRC, 'generated', 'hg_proc_*.cu')))
 
 
-def _deps():
-    out = sources() + glob.glob(os.path.join(CSRC, '*.cuh')) + glob.glob(os.path.join(CSRC, '*.h')) + \
-        glob.glob(os.path.join(CSRC, 'generated', '*.cuh')) + [os.path.join(HERE, '..', 'include', 'hg.h'),
-                                                                os.path.abspath(__file__)]
+def _common_deps():
+    return glob.glob(os.path.join(CSRC, '*.cuh')) + glob.glob(os.path.join(CSRC, '*.h')) + \
+        glob.glob(os.path.join(HERE, '..', 'include', '*.h')) + [os.path.abspath(__file__)]
+
+
+def _deps(src):
+    """Files whose change must recompile `src`: the hand-written headers, and for a per-process unit the generated
+    headers it includes (one level of #include "..." inside csrc/generated/)."""
+    out = [src] + _common_deps()
+    todo = [src]
+    while todo:
+        f = todo.pop()
+        if os.path.dirname(f) != os.path.join(CSRC, 'generated'):
+            continue
+        with open(f) as fh:
+            for line in fh:
+                if line.startswith('#include "') and '/' not in line.split('"')[1]:
+                    inc = os.path.join(CSRC, 'generated', line.split('"')[1])
+                    if os.path.exists(inc) and inc not in out:
+                        out.append(inc)
+                        todo.append(inc)
     return out
+
+
+def _obj(src):
+    return os.path.join(OBJDIR, os.path.basename(src)[:-3] + '.o')
+
+
+def _stale(src):
+    obj = _obj(src)
+    if not os.path.exists(obj):
+        return True
+    t = os.path.getmtime(obj)
+    return any(os.path.getmtime(f) > t for f in _deps(src))
 
 
 def up_to_date():
     if not os.path.exists(LIB):
         return False
     t = os.path.getmtime(LIB)
-    return all(os.path.getmtime(f) <= t for f in _deps())
+    return not any(_stale(s) or os.path.getmtime(_obj(s)) > t for s in sources())
+
+
+def _common_deps():
+    return glob.glob(os.path.join(CSRC, '*.cuh')) + glob.glob(os.path.join(CSRC, '*.h')) + \
+        glob.glob(os.path.join(HERE, '..', 'include', '*.h')) + [os.path.abspath(__file__)]
+
+
+def _deps(src):
+    """Files whose change must recompile `src`: the hand-written headers, and for a per-process unit the generated
+    headers it includes (one level of #include "..." inside csrc/generated/)."""
+    out = [src] + _common_deps()
+    todo = [src]
+    while todo:
+        f = todo.pop()
+        if os.path.dirname(f) != os.path.join(CSRC, 'generated'):
+            continue
+        with open(f) as fh:
+            for line in fh:
+                if line.startswith('#include "') and '/' not in line.split('"')[1]:
+                    inc = os.path.join(CSRC, 'generated', line.split('"')[1])
+                    if os.path.exists(inc) and inc not in out:
+                        out.append(inc)
+                        todo.append(inc)
+    return out
+
+
+def _obj(src):
+    return os.path.join(OBJDIR, os.path.basename(src)[:-3] + '.o')
+
+
+def _stale(src):
+    obj = _obj(src)
+    if not os.path.exists(obj):
+        return True
+    t = os.path.getmtime(obj)
+    return any(os.path.getmtime(f) > t for f in _deps(src))
+
+
+def up_to_date():
+    if not os.path.exists(LIB):
+        return False
+    t = os.path.getmtime(LIB)
+    return not any(_stale(s) or os.path.getmtime(_obj(s)) > t for s in sources())
 
 
 def _compile(src):
-    obj = os.path.join(OBJDIR, os.path.basename(src)[:-3] + '.o')
+    obj = _obj(src)
     cmd = ['nvcc'] + NVCC_FLAGS + ['-c', src, '-o', obj]
     r = subprocess.run(cmd, capture_output=True, text=True)
     log = r.stdout + r.stderr
@@ -49,15 +121,18 @@ def _compile(src):
 
 
 def build(force=False, verbose=False):
+    """Recompiles the translation units whose sources or headers changed, then links."""
     if not force and up_to_date():
         return LIB
     os.makedirs(OBJDIR, exist_ok=True)
+    todo = [s for s in sources() if force or _stale(s)]
     with ThreadPoolExecutor(max_workers=max(1, min(8, os.cpu_count() or 1))) as ex:
-        res = list(ex.map(_compile, sources()))
+        res = list(ex.map(_compile, todo))
     if verbose:
         for _, log in res:
             sys.stdout.write(log)
-    cmd = ['nvcc', '-shared', '-o', LIB] + [o for o, _ in res] + ['-gencode', 'arch=compute_100a,code=sm_100a']
+    cmd = ['nvcc', '-shared', '-o', LIB] + [_obj(s) for s in sources()] + \
+        ['-gencode', 'arch=compute_100a,code=sm_100a']
     r = subprocess.run(cmd, capture_output=True, text=True)
     if r.returncode != 0:
         raise RuntimeError('link failed:\n' + r.stdout + r.stderr)

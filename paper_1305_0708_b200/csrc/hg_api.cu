@@ -7,6 +7,7 @@
 #include <string>
 #include <vector>
 
+#include "../../include/hg_bench.h"
 #include "hg_couplings.h"
 #include "hg_host_setup.h"
 #include "hg_internal.h"
@@ -47,6 +48,11 @@ struct hg_ctx {
   size_t stage_bytes = 0;
   void* d_scratch = nullptr;     // phase-space points of one chunk of hg_integrate_step (staged processes)
   size_t scratch_bytes = 0;
+  const double* d_grid = nullptr;  // hg_set_grid: caller-owned [n_draws][grid_nb + 1]
+  int grid_nb = 0;
+  double* d_hist = nullptr;        // caller-owned [n_draws][grid_nb], or NULL
+  double* d_hist_partial = nullptr;  // per-block histograms of one chunk
+  size_t hist_partial_bytes = 0;
   cudaStream_t copy_stream = nullptr;   // H2D copies of hg_matrix_element_host
   cudaEvent_t ev_h2d[2] = {nullptr, nullptr}, ev_free[2] = {nullptr, nullptr};
   int profiling = 0;             // hg_set_profiling
@@ -159,6 +165,92 @@ __global__ void __launch_bounds__(256) fma_peak_kernel(T* out, int iters, T a, T
   out[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = ((x0 + x1) + (x2 + x3)) + ((x4 + x5) + (x6 + x7));
 }
 
+// ---- adaptive grid: histograms of w^2 per (variable, bin)  (reading A22; role of the BASES grid-optimisation step)
+//
+// Deterministic, no atomics: block (b, s) takes slice s of the passing events of range b (the lists compact_kernel
+// wrote for me_acc_kernel); inside a block every warp walks its share of the slice event by event with one LANE PER
+// VARIABLE, so a lane owns row `lane` of the warp's private histogram in shared memory and nobody else touches it.
+// The warps' histograms are added in warp order, the blocks' in block order (hist_finalize_kernel).
+constexpr int kHistSplit = 4;      // blocks per range
+constexpr int kHistWarps = 4;
+constexpr int kHistMaxDim = 32;    // one lane per variable
+__global__ void __launch_bounds__(32 * kHistWarps) hist_kernel(const uint8_t* __restrict__ bins,
+                                                               const double* __restrict__ w,
+                                                               const int* __restrict__ idx, const int* __restrict__ cnt,
+                                                               int64_t m, int64_t range, int ndim, int nb,
+                                                               double* __restrict__ partial) {
+  extern __shared__ double hist_sh[];   // [kHistWarps][ndim][nb + 1]
+  const int b = blockIdx.x / kHistSplit, sidx = blockIdx.x % kHistSplit;
+  const int lane = threadIdx.x & 31, wp = threadIdx.x >> 5;
+  const int row = nb + 1;
+  for (int i = threadIdx.x; i < kHistWarps * ndim * row; i += blockDim.x) hist_sh[i] = 0.0;
+  __syncthreads();
+  const int total = cnt[b];
+  const int per = (total + kHistSplit * kHistWarps - 1) / (kHistSplit * kHistWarps);
+  const int lo = (sidx * kHistWarps + wp) * per;
+  const int hi = lo + per < total ? lo + per : total;
+  const int* __restrict__ my = idx + (int64_t)b * range;
+  double* mine = hist_sh + ((size_t)wp * ndim + lane) * row;
+  if (lane < ndim) {
+    const uint8_t* __restrict__ brow = bins + (int64_t)lane * m;
+    for (int j = lo; j < hi; ++j) {
+      const int e = my[j];
+      const double x = w[e];
+      mine[brow[e]] += x * x;
+    }
+  }
+  __syncthreads();
+  double* out = partial + (size_t)blockIdx.x * ndim * nb;
+  for (int i = threadIdx.x; i < ndim * nb; i += blockDim.x) {
+    const int d = i / nb, k = i % nb;
+    double a = 0.0;
+    for (int q = 0; q < kHistWarps; ++q) a += hist_sh[((size_t)q * ndim + d) * row + k];
+    out[i] = a;
+  }
+}
+
+__global__ void hist_finalize_kernel(const double* __restrict__ partial, int nblk, int nel, double* __restrict__ hist) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= nel) return;
+  double a = 0.0;
+  for (int b = 0; b < nblk; ++b) a += partial[(size_t)b * nel + i];
+  hist[i] += a;
+}
+
+cudaError_t GridAcc::launch(const uint8_t* d_bins, const double* d_w, const int* d_idx, const int* d_cnt, int64_t m,
+                            int64_t range, int nblocks, int n_draws, cudaStream_t s) const {
+  const int nblk = nblocks * kHistSplit;
+  const size_t smem = sizeof(double) * kHistWarps * n_draws * (nb + 1);
+  if (smem > 48 * 1024) {
+    cudaError_t e = cudaFuncSetAttribute(hist_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+  }
+  hist_kernel<<<nblk, 32 * kHistWarps, smem, s>>>(d_bins, d_w, d_idx, d_cnt, m, range, n_draws, nb, d_partial);
+  const int nel = n_draws * nb;
+  hist_finalize_kernel<<<(nel + 255) / 256, 256, 0, s>>>(d_partial, nblk, nel, d_hist);
+  return cudaGetLastError();
+}
+
+// Makes the context's device current for the duration of a call and restores the caller's device afterwards
+// (include/hg.h, hg_create): two contexts on different GPUs can be used from one thread.
+struct DeviceGuard {
+  int prev = -1;
+  cudaError_t err = cudaSuccess;
+  explicit DeviceGuard(int dev) {
+    err = cudaGetDevice(&prev);
+    if (err == cudaSuccess && prev != dev) err = cudaSetDevice(dev);
+    else if (err == cudaSuccess) prev = -1;
+  }
+  ~DeviceGuard() {
+    if (prev >= 0) cudaSetDevice(prev);
+  }
+};
+#define HG_ON_DEVICE(ctx, who)                                              \
+  DeviceGuard hg_guard((ctx)->device);                                      \
+  if (hg_guard.err != cudaSuccess) return fail_cuda((ctx), hg_guard.err, who ": cudaSetDevice")
+
+static bool misaligned(const void* p, size_t al) { return ((uintptr_t)p % al) != 0; }
+
 static bool finite_pos(double x) { return isfinite(x) && x > 0.0; }
 static bool finite_nonneg(double x) { return isfinite(x) && x >= 0.0; }
 
@@ -174,7 +266,8 @@ int hg_create(hg_ctx** out, int cuda_device) {
     return HG_EINVAL;
   }
   *out = nullptr;
-  cudaError_t e = cudaSetDevice(cuda_device);
+  DeviceGuard guard(cuda_device);
+  cudaError_t e = guard.err;
   if (e != cudaSuccess) {
     g_create_error = std::string("hg_create: cudaSetDevice: ") + cudaGetErrorString(e);
     return HG_ECUDA;
@@ -199,11 +292,13 @@ int hg_create(hg_ctx** out, int cuda_device) {
 
 void hg_destroy(hg_ctx* ctx) {
   if (!ctx) return;
+  DeviceGuard guard(ctx->device);
   if (ctx->d_partials) cudaFree(ctx->d_partials);
   if (ctx->d_acc) cudaFree(ctx->d_acc);
   if (ctx->h_acc) cudaFreeHost(ctx->h_acc);
   if (ctx->d_stage) cudaFree(ctx->d_stage);
   if (ctx->d_scratch) cudaFree(ctx->d_scratch);
+  if (ctx->d_hist_partial) cudaFree(ctx->d_hist_partial);
   for (cudaEvent_t ev : ctx->ev) cudaEventDestroy(ev);
   for (int i = 0; i < 2; ++i) {
     if (ctx->ev_h2d[i]) cudaEventDestroy(ctx->ev_h2d[i]);
@@ -316,8 +411,13 @@ int hg_gen_phase_space(hg_ctx* ctx, int process, int precision, uint64_t seed, u
   if ((rc = check_rs(ctx, vt, process, sqrt_s_hat, "hg_gen_phase_space")) != HG_OK) return rc;
   if (n == 0) return HG_OK;
   if (!d_p || !d_wps) return fail(ctx, HG_EINVAL, "hg_gen_phase_space: d_p / d_wps is NULL");
+  if (misaligned(d_p, precision == HG_F64 ? 8 : 4) || misaligned(d_wps, precision == HG_F64 ? 8 : 4))
+    return fail(ctx, HG_EINVAL, "hg_gen_phase_space: misaligned pointer");
+  HG_ON_DEVICE(ctx, "hg_gen_phase_space");
   const int n_rambo = process == HG_GG_TTXG_DILEP ? 3 : vt->info.n_final;
-  const PsConst k = make_psconst(ctx->par, ctx->cuts[process], n_rambo, sqrt_s_hat);
+  PsConst k = make_psconst(ctx->par, ctx->cuts[process], n_rambo, sqrt_s_hat);
+  k.grid = ctx->d_grid;
+  k.nb = ctx->grid_nb;
   cudaError_t e = vt->ps(precision, n, k, seed, first_event, d_p, d_wps, d_pass, (cudaStream_t)cuda_stream);
   if (e != cudaSuccess) return fail_cuda(ctx, e, "hg_gen_phase_space");
   return HG_OK;
@@ -333,6 +433,7 @@ int hg_matrix_element(hg_ctx* ctx, int process, int precision, int64_t n, const 
   const size_t al = precision == HG_F64 ? 8 : 4;
   if (((uintptr_t)d_p % al) || ((uintptr_t)d_me2 % al))
     return fail(ctx, HG_EINVAL, "hg_matrix_element: misaligned pointer");
+  HG_ON_DEVICE(ctx, "hg_matrix_element");
   cudaError_t e = vt->me(precision, n, d_p, d_me2, ctx->coup, (cudaStream_t)cuda_stream);
   if (e != cudaSuccess) return fail_cuda(ctx, e, "hg_matrix_element");
   return HG_OK;
@@ -345,6 +446,9 @@ int hg_matrix_element_host(hg_ctx* ctx, int process, int precision, int64_t n, c
   if (!vt) return rc;
   if (n == 0) return HG_OK;
   if (!h_p || !h_me2) return fail(ctx, HG_EINVAL, "hg_matrix_element_host: h_p / h_me2 is NULL");
+  if (misaligned(h_p, precision == HG_F64 ? 8 : 4) || misaligned(h_me2, precision == HG_F64 ? 8 : 4))
+    return fail(ctx, HG_EINVAL, "hg_matrix_element_host: misaligned pointer");
+  HG_ON_DEVICE(ctx, "hg_matrix_element_host");
   // Pipelined in chunks of kHostChunk events over two device buffers: the H2D copy of chunk i+1 (on a context-owned
   // copy stream) overlaps the kernel and the D2H copy of chunk i (on the caller's stream).  The host array is
   // [n_ext][4][n], so one chunk is 4 n_ext strided rows: one cudaMemcpy2DAsync.
@@ -420,6 +524,9 @@ int hg_accumulate(hg_ctx* ctx, int precision, int64_t n, const void* d_me2, cons
   acc[0] = acc[1] = acc[2] = acc[3] = 0.0;
   if (n == 0) return HG_OK;
   if (!d_me2 || !d_wps) return fail(ctx, HG_EINVAL, "hg_accumulate: d_me2 / d_wps is NULL");
+  if (misaligned(d_me2, precision == HG_F64 ? 8 : 4) || misaligned(d_wps, precision == HG_F64 ? 8 : 4))
+    return fail(ctx, HG_EINVAL, "hg_accumulate: misaligned pointer");
+  HG_ON_DEVICE(ctx, "hg_accumulate");
   cudaStream_t s = (cudaStream_t)cuda_stream;
   const double wscale = kHbarC2Pb / (2.0 * sqrt_s_hat * sqrt_s_hat);
   int nblocks = ctx->n_sm * 8;
@@ -446,22 +553,27 @@ int hg_integrate_step(hg_ctx* ctx, int process, int precision, uint64_t seed, ui
   if ((rc = check_rs(ctx, vt, process, sqrt_s_hat, "hg_integrate_step")) != HG_OK) return rc;
   acc[0] = acc[1] = acc[2] = acc[3] = 0.0;
   if (n == 0) return HG_OK;
+  HG_ON_DEVICE(ctx, "hg_integrate_step");
   cudaStream_t s = (cudaStream_t)cuda_stream;
   const int n_rambo = process == HG_GG_TTXG_DILEP ? 3 : vt->info.n_final;
-  const PsConst k = make_psconst(ctx->par, ctx->cuts[process], n_rambo, sqrt_s_hat);
+  PsConst k = make_psconst(ctx->par, ctx->cuts[process], n_rambo, sqrt_s_hat);
+  k.grid = ctx->d_grid;
+  k.nb = ctx->grid_nb;
+  const bool hist = ctx->d_grid && ctx->d_hist;      // grid-optimisation step: accumulate the histograms
+  const bool split = vt->split_step() || ctx->d_grid != nullptr;   // grid sampling: always the split step
   const double wscale = kHbarC2Pb / (2.0 * sqrt_s_hat * sqrt_s_hat);
   int per_sm = 1;
-  cudaError_t e = vt->int_blocks_per_sm(precision, &per_sm);
+  cudaError_t e = vt->int_blocks_per_sm(precision, split, &per_sm);
   if (e != cudaSuccess) return fail_cuda(ctx, e, "hg_integrate_step: occupancy query");
   if (per_sm < 1) per_sm = 1;
   int nblocks = ctx->n_sm * per_sm;  // persistent grid: a whole number of resident waves
   if (nblocks > kMaxPartialBlocks) nblocks = kMaxPartialBlocks;
   const int64_t need = (n + kIntThreads - 1) / kIntThreads;
   if (need < nblocks) nblocks = (int)need;
-  const size_t per_event = vt->scratch_bytes_per_event(precision);
   const int64_t chunk = n < kIntChunk ? n : kIntChunk;
-  if (per_event) {  // two kernels per chunk through a context-owned buffer, grown on demand
-    const size_t bytes = per_event * (size_t)chunk + 1024 + sizeof(int) * kMaxPartialBlocks;
+  const bool per_event = split;
+  if (split) {  // separate kernels per chunk through a context-owned buffer, grown on demand
+    const size_t bytes = vt->scratch_bytes(precision, chunk, hist);
     if (bytes > ctx->scratch_bytes) {
       if (ctx->d_scratch) cudaFree(ctx->d_scratch);
       ctx->d_scratch = nullptr;
@@ -470,6 +582,21 @@ int hg_integrate_step(hg_ctx* ctx, int process, int precision, uint64_t seed, ui
       if (e != cudaSuccess) return fail_cuda(ctx, e, "hg_integrate_step: cudaMalloc of the chunk buffer");
       ctx->scratch_bytes = bytes;
     }
+  }
+  GridAcc ga;
+  if (hist) {
+    const size_t bytes = sizeof(double) * (size_t)nblocks * kHistSplit * vt->info.n_draws * ctx->grid_nb;
+    if (bytes > ctx->hist_partial_bytes) {
+      if (ctx->d_hist_partial) cudaFree(ctx->d_hist_partial);
+      ctx->d_hist_partial = nullptr;
+      ctx->hist_partial_bytes = 0;
+      e = cudaMalloc(&ctx->d_hist_partial, bytes);
+      if (e != cudaSuccess) return fail_cuda(ctx, e, "hg_integrate_step: cudaMalloc of the histogram partials");
+      ctx->hist_partial_bytes = bytes;
+    }
+    ga.nb = ctx->grid_nb;
+    ga.d_partial = ctx->d_hist_partial;
+    ga.d_hist = ctx->d_hist;
   }
   const int nchunks = per_event ? (int)((n + chunk - 1) / chunk) : 1;
   cudaEvent_t* ev = nullptr;
@@ -482,9 +609,9 @@ int hg_integrate_step(hg_ctx* ctx, int process, int precision, uint64_t seed, ui
     ev = ctx->ev.data();
   }
   e = vt->integrate(precision, n, k, seed, first_event, ctx->coup, wscale, ctx->d_partials, nblocks, ctx->d_scratch,
-                    chunk, ev, s);
+                    chunk, ev, hist ? &ga : nullptr, s);
   if (e != cudaSuccess) return fail_cuda(ctx, e, "hg_integrate_step");
-  ctx->n_launches = (per_event ? 3 * nchunks : 1) + 1;
+  ctx->n_launches = (per_event ? (hist ? 5 : 3) * nchunks : 1) + 1;
   rc = finish(ctx, nblocks, n, acc, s, "hg_integrate_step");  // synchronises the stream
   if (rc == HG_OK && ev) {
     ctx->t_ps_ms = ctx->t_me_ms = 0;
@@ -501,6 +628,75 @@ int hg_integrate_step(hg_ctx* ctx, int process, int precision, uint64_t seed, ui
     }
   }
   return rc;
+}
+
+int hg_set_grid(hg_ctx* ctx, const double* d_grid, int n_bins, double* d_hist) {
+  if (!ctx) return HG_EINVAL;
+  if (!d_grid) {
+    ctx->d_grid = nullptr;
+    ctx->grid_nb = 0;
+    ctx->d_hist = nullptr;
+    return HG_OK;
+  }
+  if (n_bins < 2 || n_bins > HG_GRID_MAX_BINS) return fail(ctx, HG_EINVAL, "hg_set_grid: n_bins out of range");
+  if (misaligned(d_grid, 8) || misaligned(d_hist, 8)) return fail(ctx, HG_EINVAL, "hg_set_grid: misaligned pointer");
+  ctx->d_grid = d_grid;
+  ctx->grid_nb = n_bins;
+  ctx->d_hist = d_hist;
+  return HG_OK;
+}
+
+int hg_grid_refine(int n_dim, int n_bins, const double* h_hist, double alpha, double* h_grid) {
+  if (n_dim < 1 || n_bins < 2 || n_bins > HG_GRID_MAX_BINS || !h_hist || !h_grid || !(alpha >= 0.0)) return HG_EINVAL;
+  const int nb = n_bins;
+  std::vector<double> sm(nb), r(nb), edges(nb + 1);
+  for (int d = 0; d < n_dim; ++d) {
+    const double* h = h_hist + (size_t)d * nb;
+    double* g = h_grid + (size_t)d * (nb + 1);
+    double tot = 0.0;
+    bool fin = true;
+    for (int i = 0; i < nb; ++i) {
+      fin = fin && isfinite(h[i]);
+      tot += h[i];
+    }
+    if (!fin || !(tot > 0.0)) continue;            // nothing accumulated for this variable: grid unchanged
+    // smoothing over neighbouring bins, normalisation
+    sm[0] = (h[0] + h[1]) / 2.0;
+    sm[nb - 1] = (h[nb - 2] + h[nb - 1]) / 2.0;
+    for (int i = 1; i < nb - 1; ++i) sm[i] = (h[i - 1] + h[i] + h[i + 1]) / 3.0;
+    double ssum = 0.0;
+    for (int i = 0; i < nb; ++i) ssum += sm[i];
+    // compression r = ((1 - s) / ln(1 / s))^alpha
+    double rsum = 0.0;
+    for (int i = 0; i < nb; ++i) {
+      const double x = sm[i] / ssum;
+      r[i] = 0.0;
+      if (x > 0.0) r[i] = x >= 1.0 ? 1.0 : pow((1.0 - x) / log(1.0 / x), alpha);
+      rsum += r[i];
+    }
+    const double per = rsum / nb;
+    if (!(per > 0.0)) continue;
+    // new edges: every new bin holds `per`, r spread evenly inside an old bin
+    edges[0] = 0.0;
+    edges[nb] = 1.0;
+    int k = 0;
+    double acc = 0.0;
+    for (int j = 1; j < nb; ++j) {
+      const double target = j * per;
+      while (k < nb - 1 && acc + r[k] < target) {
+        acc += r[k];
+        ++k;
+      }
+      double frac = r[k] > 0.0 ? (target - acc) / r[k] : 0.0;
+      frac = frac < 0.0 ? 0.0 : (frac > 1.0 ? 1.0 : frac);
+      edges[j] = g[k] + frac * (g[k + 1] - g[k]);
+    }
+    for (int j = 1; j <= nb; ++j)
+      if (!(edges[j] > edges[j - 1])) edges[j] = nextafter(edges[j - 1], 2.0);
+    edges[nb] = 1.0;
+    for (int j = 0; j <= nb; ++j) g[j] = edges[j];
+  }
+  return HG_OK;
 }
 
 int hg_set_profiling(hg_ctx* ctx, int on) {
@@ -521,6 +717,7 @@ int hg_measure_fma_peak(hg_ctx* ctx, int precision, double* flops_per_s, void* c
   if (!ctx) return HG_EINVAL;
   if (!flops_per_s) return fail(ctx, HG_EINVAL, "hg_measure_fma_peak: flops_per_s is NULL");
   if (precision != HG_F64 && precision != HG_F32) return fail(ctx, HG_EINVAL, "hg_measure_fma_peak: unknown precision");
+  HG_ON_DEVICE(ctx, "hg_measure_fma_peak");
   cudaStream_t s = (cudaStream_t)cuda_stream;
   const int blocks = ctx->n_sm * 8, threads = 256, iters = precision == HG_F64 ? 4096 : 8192;
   void* d_out = nullptr;

@@ -57,6 +57,8 @@ inline PsConst make_psconst(const hg_params& par, const hg_cuts& cuts, int n_ram
   k.eta_jet_max = cuts.eta_jet_max;
   k.eta_lep_max = cuts.eta_lep_max;
   k.dr_jj_min = cuts.dr_jj_min;
+  k.grid = nullptr;
+  k.nb = 0;
   return k;
 }
 

@@ -18,6 +18,16 @@ constexpr int64_t kIntChunk = (int64_t)1 << 20;
 // events per chunk of the copy/compute pipeline of hg_matrix_element_host
 constexpr int64_t kHostChunk = (int64_t)1 << 19;
 
+// Accumulation of the adaptive-grid histograms after a chunk of the split step (hg_api.cu: hist_kernel): for the
+// passing events listed by (idx, cnt, range, nblocks) adds w^2 into the bin of every draw.
+struct GridAcc {
+  int nb;               // bins per variable
+  double* d_partial;    // [blocks][n_draws][nb] per-block histograms
+  double* d_hist;       // [n_draws][nb], caller-owned, added to
+  cudaError_t launch(const uint8_t* d_bins, const double* d_w, const int* d_idx, const int* d_cnt, int64_t m,
+                     int64_t range, int nblocks, int n_draws, cudaStream_t s) const;
+};
+
 struct ProcVTable {
   hg_process_info_t info;
   // hg_matrix_element: p [n_ext][4][n] -> me2 [n]
@@ -28,15 +38,18 @@ struct ProcVTable {
   // hg_integrate_step: writes nblocks x (sum w, sum w^2, n_pass) partials; wscale = (hbar c)^2 / (2 s_hat)
   // ev (or NULL): 3 events per chunk, recorded on s before the phase-space kernel, between the two kernels and
   // after the matrix-element kernel (hg_set_profiling); a fused process records ev[0] and ev[2] around its kernel.
-  // Staged processes (scratch_bytes_per_event > 0) run the step as two kernels per chunk of `chunk` events
-  // through the caller's scratch buffer (momenta, weight, pass flag); the others ignore scratch and chunk.
+  // Split-step processes (and every process when ga != NULL) run the step as separate kernels per chunk of `chunk`
+  // events through the caller's scratch buffer (momenta, weight, pass flag, ...); the others ignore scratch and chunk.
+  // ga (or NULL): adaptive-grid step, histograms accumulated after each chunk.
   cudaError_t (*integrate)(int prec, int64_t n, const PsConst& k, uint64_t seed, uint64_t first,
                            const Coup<double>& c, double wscale, double* d_partials, int nblocks,
-                           void* d_scratch, int64_t chunk, cudaEvent_t* ev, cudaStream_t s);
-  // resident blocks per SM of the fused kernel for this precision (occupancy query)
-  cudaError_t (*int_blocks_per_sm)(int prec, int* out);
-  // bytes of scratch per event of a chunk for the given precision (0: the step is one fused kernel)
-  size_t (*scratch_bytes_per_event)(int prec);
+                           void* d_scratch, int64_t chunk, cudaEvent_t* ev, const GridAcc* ga, cudaStream_t s);
+  // resident blocks per SM of the kernel that evaluates the matrix element in the step (occupancy query); split:
+  // the split step is forced (adaptive-grid steps run every process as separate kernels)
+  cudaError_t (*int_blocks_per_sm)(int prec, bool split, int* out);
+  // bytes of the chunk buffer of the split step for `chunk` events; grid: with the histogram sections
+  size_t (*scratch_bytes)(int prec, int64_t chunk, bool grid);
+  bool (*split_step)();
 };
 
 extern const ProcVTable hg_proc_1, hg_proc_2, hg_proc_3, hg_proc_4, hg_proc_5, hg_proc_6, hg_proc_7, hg_proc_8, hg_proc_9;

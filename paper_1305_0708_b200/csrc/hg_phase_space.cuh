@@ -40,7 +40,34 @@ struct PsConst {
   double mh;       // Higgs mass (final-state mass of the Higgs-sector processes)
   double tmax_t, tmax_w;  // atan(min(20, m/Gamma))  (A.15; reading A14)
   double pt_jet_min, eta_jet_max, eta_lep_max, dr_jj_min;  // cuts, <= 0 disables
+  // adaptive grid of the integration step (hg_set_grid, reading A22): device array [n_draws][nb + 1] of bin edges in
+  // [0, 1], or NULL for flat sampling
+  const double* grid;
+  int nb;
 };
+
+// Grid-optimised sampling (role of the BASES grid; VEGAS algorithm, reading A22):
+// uniform y picks bin i = floor(y nb) of variable d and the point x = g[i] + (y nb - i)(g[i+1] - g[i]) in it; the
+// Jacobian is nb (g[i+1] - g[i]).  u is mapped in place; returns the product of the Jacobians; bins (if not NULL)
+// receives the bin of every variable.  x stays strictly below 1 (RAMBO takes log x).
+template <int ND>
+HG_HD double grid_map(const PsConst& k, double* u, uint8_t* bins) {
+  double jac = 1.0;
+  const int nb = k.nb;
+#pragma unroll
+  for (int d = 0; d < ND; ++d) {
+    const double t = u[d] * (double)nb;
+    int i = (int)t;
+    if (i > nb - 1) i = nb - 1;
+    const double* g = k.grid + (size_t)d * (nb + 1) + i;
+    const double lo = g[0], w = g[1] - lo;
+    const double x = lo + (t - (double)i) * w;
+    u[d] = x < 0.99999999999999988898 ? x : 0.99999999999999988898;  // 1 - 2^-53
+    jac *= (double)nb * w;
+    if (bins) bins[d] = (uint8_t)i;
+  }
+  return jac;
+}
 
 // isotropic massless momentum of energy e
 HG_HD Mom<double> iso(double uc, double uf, double e) {
@@ -181,23 +208,29 @@ HG_HD double two_body(const Mom<double>& P, double M2, double m1sq, double m2sq,
 
 // ---------------------------------------------------------------- per-process generators
 // Writes p[0..n_ext) (leg order of include/hg.h) and returns the phase-space weight.
-template <int NFINAL>
-HG_HD double gen_massless(const PsConst& k, uint64_t seed, uint64_t event, uint32_t pid, Mom<double>* p) {
+// GRID: the call samples through the adaptive grid k.grid (compile-time, so that the flat kernels carry none of it)
+template <int NFINAL, bool GRID>
+HG_HD double gen_massless(const PsConst& k, uint64_t seed, uint64_t event, uint32_t pid, Mom<double>* p,
+                          uint8_t* bins) {
   double u[4 * NFINAL];
   draw_uniforms<4 * NFINAL>(seed, event, pid, u);
+  double jac = 1.0;
+  if constexpr (GRID) jac = grid_map<4 * NFINAL>(k, u, bins);
   const double h = 0.5 * k.rs;
   p[0] = mkmom<double>(h, 0.0, 0.0, h);
   p[1] = mkmom<double>(h, 0.0, 0.0, -h);
   rambo_massless<NFINAL>(u, k.rs, p + 2);
-  return k.vol;
+  return k.vol * jac;
 }
 
 // Final states with massive particles (Higgs-sector processes): massive RAMBO, masses m[i] of the final legs.
-template <int NFINAL>
+template <int NFINAL, bool GRID>
 HG_HD double gen_massive(const PsConst& k, uint64_t seed, uint64_t event, uint32_t pid, const double (&m)[NFINAL],
-                         Mom<double>* p) {
+                         Mom<double>* p, uint8_t* bins) {
   double u[4 * NFINAL];
   draw_uniforms<4 * NFINAL>(seed, event, pid, u);
+  double jac = 1.0;
+  if constexpr (GRID) jac = grid_map<4 * NFINAL>(k, u, bins);
   const double h = 0.5 * k.rs;
   p[0] = mkmom<double>(h, 0.0, 0.0, h);
   p[1] = mkmom<double>(h, 0.0, 0.0, -h);
@@ -207,19 +240,23 @@ HG_HD double gen_massive(const PsConst& k, uint64_t seed, uint64_t event, uint32
     m2[i] = m[i] * m[i];
     msum += m[i];
   }
-  return k.vol * rambo_massive<NFINAL>(u, m2, msum, k.rs, p + 2);
+  return k.vol * jac * rambo_massive<NFINAL>(u, m2, msum, k.rs, p + 2);
 }
 
 // config 4: g g -> (t -> b (W+ -> e+ ve)) (t~ -> b~ (W- -> mu- vm~)) g.  Draws: 0-3 s_t, s_t~, s_W+, s_W-;
 // 4-15 RAMBO(t*, t~*, g); 16,17 t* decay angles; 18,19 W+*; 20,21 t~*; 22,23 W-*.
-HG_HD double gen_ttxg_dilep(const PsConst& k, uint64_t seed, uint64_t event, uint32_t pid, Mom<double>* p) {
+template <bool GRID>
+HG_HD double gen_ttxg_dilep(const PsConst& k, uint64_t seed, uint64_t event, uint32_t pid, Mom<double>* p,
+                            uint8_t* bins) {
   double u[24];
   draw_uniforms<24>(seed, event, pid, u);
+  double jac = 1.0;
+  if constexpr (GRID) jac = grid_map<24>(k, u, bins);
   const double h = 0.5 * k.rs;
   p[0] = mkmom<double>(h, 0.0, 0.0, h);
   p[1] = mkmom<double>(h, 0.0, 0.0, -h);
   double st, stb, swp, swm;
-  double w = bw_mass(u[0], k.mt, k.mgt, k.tmax_t, st);
+  double w = jac * bw_mass(u[0], k.mt, k.mgt, k.tmax_t, st);
   w *= bw_mass(u[1], k.mt, k.mgt, k.tmax_t, stb);
   w *= bw_mass(u[2], k.mw, k.mgw, k.tmax_w, swp);
   w *= bw_mass(u[3], k.mw, k.mgw, k.tmax_w, swm);

@@ -3,13 +3,15 @@
 // P is the generated process descriptor: n_ext, n_final, pid, jets/leptons for the cuts, gen() (phase space),
 // me2<T>() (the fused helicity+colour summed matrix element emitted by gen/emit.py).
 //
-// Design: one phase-space point per thread, as in the paper, but
-//   * a single fused kernel per process (the paper splits long amplitudes into several kernels with state in
+// Design: one phase-space point per thread, as in the paper -- or per
+// pair of warps for the staged processes -- and
+//   * one matrix-element kernel per process (the paper splits long amplitudes into several kernels with state in
 //     global memory, PAPER.md:669 -- a CUDA 4.2 limit, not needed here);
 //   * momenta in HBM are structure-of-arrays p[leg][mu][event]: a warp reads 32 consecutive values per
-//     component (one or two full 128-byte lines), every wavefunction lives in registers;
-//   * hg_integrate_step never touches HBM per event: Philox -> momenta -> cuts -> |M|^2 -> weight stay in
-//     registers, the block reduces (sum w, sum w^2, n_pass) with warp shuffles and writes one partial.
+//     component (one or two full 128-byte lines), every wavefunction lives in registers or the staging area;
+//   * hg_integrate_step is one fused kernel (integrate_kernel: nothing per event touches HBM) for the small
+//     processes, and per chunk a phase-space kernel, an ordered compaction and me_acc_kernel for the others
+//     (P::split_step); the block reduces (sum w, sum w^2, n_pass) with warp shuffles and writes one partial.
 #pragma once
 #include "hg_internal.h"
 #include "hg_stage.cuh"
@@ -88,23 +90,36 @@ __global__ void __launch_bounds__(THREADS) me_kernel(const T* __restrict__ p, T*
   if (e0 < n && ev_owner<P>()) me2[e0] = r;
 }
 
-template <class P, class T, class W>
+// BEAMS = true: all n_ext legs are written (hg_gen_phase_space).  BEAMS = false (chunk buffer of the split step): only
+// the final-state legs, leg l at row l - 2; the two incoming momenta are sqrt(s_hat)/2 (1, 0, 0, +-1) for every
+// event and me_acc_kernel rebuilds them from its arguments (64 of the 224 + 9 bytes per event of W + 3 jets less
+// to write and read back).  bins (or NULL): [n_draws][n] grid bins of the draws (adaptive-grid steps).
+// GRID: sampling through the adaptive grid k.grid (a separate instantiation: the flat kernel keeps its 72 registers).
+template <class P, class T, class W, bool BEAMS, bool GRID>
 __global__ void __launch_bounds__(128) ps_kernel(const PsConst k, uint64_t seed, uint64_t first, int64_t n,
                                                  T* __restrict__ p, W* __restrict__ wps,
-                                                 uint8_t* __restrict__ pass) {
+                                                 uint8_t* __restrict__ pass, uint8_t* __restrict__ bins) {
   const int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (e >= n) return;
   Mom<double> q[P::n_ext];
-  const double w = P::gen(k, seed, first + (uint64_t)e, q);
+  uint8_t b[GRID ? P::n_draws : 1];
+  const double w = P::template gen<GRID>(k, seed, first + (uint64_t)e, q, GRID && bins ? b : nullptr);
+  constexpr int L0 = BEAMS ? 0 : 2;
 #pragma unroll
-  for (int l = 0; l < P::n_ext; ++l) {
-    p[(l * 4 + 0) * n + e] = T(q[l].e);
-    p[(l * 4 + 1) * n + e] = T(q[l].x);
-    p[(l * 4 + 2) * n + e] = T(q[l].y);
-    p[(l * 4 + 3) * n + e] = T(q[l].z);
+  for (int l = L0; l < P::n_ext; ++l) {
+    p[((l - L0) * 4 + 0) * n + e] = T(q[l].e);
+    p[((l - L0) * 4 + 1) * n + e] = T(q[l].x);
+    p[((l - L0) * 4 + 2) * n + e] = T(q[l].y);
+    p[((l - L0) * 4 + 3) * n + e] = T(q[l].z);
   }
   wps[e] = W(w);
   if (pass) pass[e] = passes_cuts<P>(k, q) ? 1 : 0;
+  if constexpr (GRID) {
+    if (bins) {
+#pragma unroll
+      for (int d = 0; d < P::n_draws; ++d) bins[(int64_t)d * n + e] = b[d];
+    }
+  }
 }
 
 // Block reduction of three doubles: warp shuffle, then one value per warp through shared memory.
@@ -136,10 +151,13 @@ __device__ __forceinline__ void block_reduce3(double& a, double& b, double& c) {
   }
 }
 
+// me2_event of a staged process holds block-wide rendezvous, so it cannot sit under the divergent `if (passes_cuts)`
+// below: staged processes always take the split step.
 template <class P, class T, int THREADS>
 __global__ void __launch_bounds__(THREADS) integrate_kernel(const PsConst k, uint64_t seed, uint64_t first,
                                                                 int64_t n, const Coup<T> c, double wscale,
                                                                 double* __restrict__ partials) {
+  static_assert(P::n_stage == 0 || P::split_step, "a staged matrix element needs the split step");
   double sw = 0.0, sw2 = 0.0, np = 0.0;
   const int64_t stride = (int64_t)gridDim.x * blockDim.x;
   for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < n; e += stride) {
@@ -201,11 +219,14 @@ static __global__ void __launch_bounds__(256) compact_kernel(const uint8_t* __re
 // kernels because the phase-space code wants ~70 registers at full occupancy while the staged matrix element
 // runs at 5-6 warps per SM; the round trip through HBM is 32 n_ext + 9 bytes per event against >= 2e4 flops.
 // A block skips me2 only if none of its events passes (every thread must reach the rendezvous inside me2).
+// p holds the final-state legs only (ps_kernel<.., BEAMS = false>); ebeam = sqrt(s_hat)/2.  wout (or NULL): receives
+// the final weight w [pb] of every passing event at its index (adaptive-grid steps: input of hist_kernel).
 template <class P, class T, int THREADS>
 __global__ void __launch_bounds__(THREADS) me_acc_kernel(const T* __restrict__ p, const double* __restrict__ wps,
                                                          const int* __restrict__ idx, const int* __restrict__ cnt,
                                                          int64_t n, int64_t range, const Coup<T> c, double wscale,
-                                                         int add, double* __restrict__ partials) {
+                                                         double ebeam, int add, double* __restrict__ partials,
+                                                         double* __restrict__ wout) {
   constexpr int EPB = THREADS / kSplit<P>;
   double sw = 0.0, sw2 = 0.0, np = 0.0;
   const int m = cnt[blockIdx.x];                    // passing events of this block's range, block-uniform
@@ -215,15 +236,18 @@ __global__ void __launch_bounds__(THREADS) me_acc_kernel(const T* __restrict__ p
     const bool ok = j < m;
     const int64_t e = my[ok ? j : m - 1];           // tail lanes recompute the last event (rendezvous inside me2)
     Mom<T> q[P::n_ext];
+    q[0] = mkmom<T>(T(ebeam), T(0), T(0), T(ebeam));
+    q[1] = mkmom<T>(T(ebeam), T(0), T(0), T(-ebeam));
 #pragma unroll
-    for (int l = 0; l < P::n_ext; ++l)
-      q[l] = mkmom<T>(p[(l * 4 + 0) * n + e], p[(l * 4 + 1) * n + e], p[(l * 4 + 2) * n + e],
-                      p[(l * 4 + 3) * n + e]);
+    for (int l = 2; l < P::n_ext; ++l)
+      q[l] = mkmom<T>(p[((l - 2) * 4 + 0) * n + e], p[((l - 2) * 4 + 1) * n + e], p[((l - 2) * 4 + 2) * n + e],
+                      p[((l - 2) * 4 + 3) * n + e]);
     const double w = (double)me2_event<P, T, THREADS>(q, c) * wps[e] * wscale;
     if (ok && ev_owner<P>()) {
       sw += w;
       sw2 += w * w;
       np += 1.0;
+      if (wout) wout[e] = w;
     }
   }
   block_reduce3(sw, sw2, np);
@@ -269,78 +293,116 @@ struct Launch {
   static cudaError_t ps(int prec, int64_t n, const PsConst& k, uint64_t seed, uint64_t first, void* d_p,
                         void* d_wps, uint8_t* d_pass, cudaStream_t s) {
     const unsigned grid = (unsigned)((n + 127) / 128);
-    if (prec == HG_F64)
-      ps_kernel<P, double, double><<<grid, 128, 0, s>>>(k, seed, first, n, (double*)d_p, (double*)d_wps, d_pass);
-    else
-      ps_kernel<P, float, float><<<grid, 128, 0, s>>>(k, seed, first, n, (float*)d_p, (float*)d_wps, d_pass);
+    if (prec == HG_F64) {
+      if (k.grid)
+        ps_kernel<P, double, double, true, true><<<grid, 128, 0, s>>>(k, seed, first, n, (double*)d_p,
+                                                                      (double*)d_wps, d_pass, nullptr);
+      else
+        ps_kernel<P, double, double, true, false><<<grid, 128, 0, s>>>(k, seed, first, n, (double*)d_p,
+                                                                       (double*)d_wps, d_pass, nullptr);
+    } else {
+      if (k.grid)
+        ps_kernel<P, float, float, true, true><<<grid, 128, 0, s>>>(k, seed, first, n, (float*)d_p, (float*)d_wps,
+                                                                    d_pass, nullptr);
+      else
+        ps_kernel<P, float, float, true, false><<<grid, 128, 0, s>>>(k, seed, first, n, (float*)d_p, (float*)d_wps,
+                                                                     d_pass, nullptr);
+    }
     return cudaGetLastError();
+  }
+  // Layout of the chunk buffer of the split step (context-owned, hg_api.cu): final-state momenta [n_ext - 2][4][chunk]
+  // of T | weight double[chunk] | index list int[chunk] | per-block counts int[kMaxPartialBlocks] | pass flags
+  // u8[chunk] | adaptive-grid steps only: final weights double[chunk], grid bins u8[n_draws][chunk].
+  struct Scratch {   // byte offsets of the sections, each 256-byte aligned
+    size_t p, w, idx, cnt, ok, wout, bins, total;
+  };
+  static Scratch scratch_layout(size_t el, int64_t chunk, bool grid) {
+    auto up = [](size_t x) { return (x + 255) / 256 * 256; };
+    Scratch L;
+    L.p = 0;
+    L.w = up((size_t)chunk * (P::n_ext - 2) * 4 * el);
+    L.idx = L.w + up((size_t)chunk * 8);
+    L.cnt = L.idx + up((size_t)chunk * 4);
+    L.ok = L.cnt + up(sizeof(int) * kMaxPartialBlocks);
+    L.wout = L.ok + up((size_t)chunk);
+    L.bins = L.wout + (grid ? up((size_t)chunk * 8) : 0);
+    L.total = L.bins + (grid ? up((size_t)chunk * P::n_draws) : 0);
+    return L;
+  }
+  static size_t scratch_bytes(int prec, int64_t chunk, bool grid) {
+    return scratch_layout(prec == HG_F64 ? 8 : 4, chunk, grid).total;
   }
   template <class T>
   static cudaError_t integrate_t(int64_t n, const PsConst& k, uint64_t seed, uint64_t first, const Coup<T>& c,
                                  double wscale, double* d_partials, int nblocks, void* d_scratch, int64_t chunk,
-                                 cudaEvent_t* ev, cudaStream_t s) {
+                                 cudaEvent_t* ev, const GridAcc* ga, cudaStream_t s) {
     constexpr int TH = int_thr<T>();
     constexpr size_t smem = stage_bytes<P, T, TH>();
     if constexpr (!P::split_step) {
-      if (ev) cudaEventRecord(ev[0], s);
-      integrate_kernel<P, T, TH><<<nblocks, TH, smem, s>>>(k, seed, first, n, c, wscale, d_partials);
-      if (ev) cudaEventRecord(ev[2], s);
-      return cudaGetLastError();
-    } else {
-      cudaError_t err = allow_smem(me_acc_kernel<P, T, TH>, smem);
-      if (err != cudaSuccess) return err;
-      for (int64_t off = 0; off < n; off += chunk) {
-        const int64_t m = n - off < chunk ? n - off : chunk;
-        T* d_p = (T*)d_scratch;                                      // [n_ext][4][m]
-        double* d_w = (double*)((char*)d_scratch + scratch_p_bytes<T>(chunk));
-        int* d_idx = (int*)(d_w + chunk);
-        int* d_cnt = d_idx + chunk;
-        uint8_t* d_ok = (uint8_t*)(d_cnt + kMaxPartialBlocks);
-        const int64_t range = (m + nblocks - 1) / nblocks;
-        cudaEvent_t* e3 = ev ? ev + 3 * (off / chunk) : nullptr;
-        if (e3) cudaEventRecord(e3[0], s);
-        ps_kernel<P, T, double><<<(unsigned)((m + 127) / 128), 128, 0, s>>>(k, seed, first + (uint64_t)off, m, d_p,
-                                                                            d_w, d_ok);
-        compact_kernel<<<nblocks, 256, 0, s>>>(d_ok, m, range, d_idx, d_cnt);
-        if (e3) cudaEventRecord(e3[1], s);
-        me_acc_kernel<P, T, TH><<<nblocks, TH, smem, s>>>(d_p, d_w, d_idx, d_cnt, m, range, c, wscale,
-                                                          off > 0 ? 1 : 0, d_partials);
-        if (e3) cudaEventRecord(e3[2], s);
+      if (!k.grid) {   // sampling through a grid always takes the split step (the fused kernel carries no grid code)
+        if (ev) cudaEventRecord(ev[0], s);
+        integrate_kernel<P, T, TH><<<nblocks, TH, smem, s>>>(k, seed, first, n, c, wscale, d_partials);
+        if (ev) cudaEventRecord(ev[2], s);
+        return cudaGetLastError();
       }
-      return cudaGetLastError();
     }
-  }
-  template <class T>
-  static constexpr size_t scratch_p_bytes(int64_t chunk) {
-    return ((size_t)chunk * P::n_ext * 4 * sizeof(T) + 255) / 256 * 256;
-  }
-  static size_t scratch_bytes_per_event(int prec) {
-    if (!P::split_step) return 0;
-    return (size_t)P::n_ext * 4 * (prec == HG_F64 ? 8 : 4) + 8 + 4 + 1;  // momenta, weight, index, pass flag
+    cudaError_t err = allow_smem(me_acc_kernel<P, T, TH>, smem);
+    if (err != cudaSuccess) return err;
+    char* base = (char*)d_scratch;
+    const Scratch L = scratch_layout(sizeof(T), chunk, ga != nullptr);
+    T* d_p = (T*)(base + L.p);                                     // [n_ext - 2][4][m]
+    double* d_w = (double*)(base + L.w);
+    int* d_idx = (int*)(base + L.idx);
+    int* d_cnt = (int*)(base + L.cnt);
+    uint8_t* d_ok = (uint8_t*)(base + L.ok);
+    double* d_wout = ga ? (double*)(base + L.wout) : nullptr;
+    uint8_t* d_bins = ga ? (uint8_t*)(base + L.bins) : nullptr;
+    for (int64_t off = 0; off < n; off += chunk) {
+      const int64_t m = n - off < chunk ? n - off : chunk;
+      const int64_t range = (m + nblocks - 1) / nblocks;
+      cudaEvent_t* e3 = ev ? ev + 3 * (off / chunk) : nullptr;
+      if (e3) cudaEventRecord(e3[0], s);
+      if (k.grid)
+        ps_kernel<P, T, double, false, true><<<(unsigned)((m + 127) / 128), 128, 0, s>>>(
+            k, seed, first + (uint64_t)off, m, d_p, d_w, d_ok, d_bins);
+      else
+        ps_kernel<P, T, double, false, false><<<(unsigned)((m + 127) / 128), 128, 0, s>>>(
+            k, seed, first + (uint64_t)off, m, d_p, d_w, d_ok, d_bins);
+      compact_kernel<<<nblocks, 256, 0, s>>>(d_ok, m, range, d_idx, d_cnt);
+      if (e3) cudaEventRecord(e3[1], s);
+      me_acc_kernel<P, T, TH><<<nblocks, TH, smem, s>>>(d_p, d_w, d_idx, d_cnt, m, range, c, wscale, 0.5 * k.rs,
+                                                        off > 0 ? 1 : 0, d_partials, d_wout);
+      if (e3) cudaEventRecord(e3[2], s);
+      if (ga) {
+        err = ga->launch(d_bins, d_wout, d_idx, d_cnt, m, range, nblocks, P::n_draws, s);
+        if (err != cudaSuccess) return err;
+      }
+    }
+    return cudaGetLastError();
   }
   static cudaError_t integrate(int prec, int64_t n, const PsConst& k, uint64_t seed, uint64_t first,
                                const Coup<double>& c, double wscale, double* d_partials, int nblocks,
-                               void* d_scratch, int64_t chunk, cudaEvent_t* ev, cudaStream_t s) {
+                               void* d_scratch, int64_t chunk, cudaEvent_t* ev, const GridAcc* ga, cudaStream_t s) {
     if (prec == HG_F64)
-      return integrate_t<double>(n, k, seed, first, c, wscale, d_partials, nblocks, d_scratch, chunk, ev, s);
+      return integrate_t<double>(n, k, seed, first, c, wscale, d_partials, nblocks, d_scratch, chunk, ev, ga, s);
     return integrate_t<float>(n, k, seed, first, coup_cast<float>(c), wscale, d_partials, nblocks, d_scratch, chunk,
-                              ev, s);
+                              ev, ga, s);
   }
   template <class T>
-  static cudaError_t int_blocks_t(int* out) {
+  static cudaError_t int_blocks_t(int* out, bool split) {
     constexpr int TH = int_thr<T>();
     constexpr size_t smem = stage_bytes<P, T, TH>();
     if constexpr (!P::split_step) {
-      return cudaOccupancyMaxActiveBlocksPerMultiprocessor(out, integrate_kernel<P, T, TH>, TH, smem);
-    } else {
-      cudaError_t err = allow_smem(me_acc_kernel<P, T, TH>, smem);
-      if (err != cudaSuccess) return err;
-      return cudaOccupancyMaxActiveBlocksPerMultiprocessor(out, me_acc_kernel<P, T, TH>, TH, smem);
+      if (!split) return cudaOccupancyMaxActiveBlocksPerMultiprocessor(out, integrate_kernel<P, T, TH>, TH, smem);
     }
+    cudaError_t err = allow_smem(me_acc_kernel<P, T, TH>, smem);
+    if (err != cudaSuccess) return err;
+    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(out, me_acc_kernel<P, T, TH>, TH, smem);
   }
-  static cudaError_t int_blocks_per_sm(int prec, int* out) {
-    return prec == HG_F64 ? int_blocks_t<double>(out) : int_blocks_t<float>(out);
+  static cudaError_t int_blocks_per_sm(int prec, bool split, int* out) {
+    return prec == HG_F64 ? int_blocks_t<double>(out, split) : int_blocks_t<float>(out, split);
   }
+  static bool split_step() { return P::split_step; }
 };
 
 template <class P>
@@ -348,7 +410,7 @@ constexpr ProcVTable make_vtable(double flops_me, double flops_ps) {
   return ProcVTable{hg_process_info_t{P::n_ext, P::n_final, P::n_hel_total, P::n_hel_nonzero, P::n_diagrams,
                                       P::n_amplitudes, P::n_flows, P::n_draws, P::avg_factor, flops_me, flops_ps},
                     &Launch<P>::me, &Launch<P>::ps, &Launch<P>::integrate, &Launch<P>::int_blocks_per_sm,
-                    &Launch<P>::scratch_bytes_per_event};
+                    &Launch<P>::scratch_bytes, &Launch<P>::split_step};
 }
 
 }  // namespace hg

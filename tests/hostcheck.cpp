@@ -1,22 +1,22 @@
-// hostcheck.cpp -- build-time / test tool of the generator: evaluates the generated matrix elements in fp64 on the
+// hostcheck.cpp -- test harness (tests/test_generated_host.py): evaluates the generated matrix elements in fp64 on the
 // HOST (the device library compiles as plain C++) for momenta read from stdin, so that the emitted code can be
 // checked without a GPU (tests/test_generated_host.py).  Never linked into libhg.so.
 //   input : lines "pid  E px py pz  E px py pz ..." (n_ext momenta, leg order of include/hg.h)
 //   output: one line per input line, |Mbar|^2 with 17 significant digits
 #include <stdio.h>
 
-#include "flopcount.h"
-#include "../csrc/hg_couplings.h"
-#include "../csrc/hg_host_setup.h"
-#include "../csrc/generated/hg_proc_1.cuh"
-#include "../csrc/generated/hg_proc_2.cuh"
-#include "../csrc/generated/hg_proc_3.cuh"
-#include "../csrc/generated/hg_proc_4.cuh"
-#include "../csrc/generated/hg_proc_5.cuh"
-#include "../csrc/generated/hg_proc_6.cuh"
-#include "../csrc/generated/hg_proc_7.cuh"
-#include "../csrc/generated/hg_proc_8.cuh"
-#include "../csrc/generated/hg_proc_9.cuh"
+#include "../paper_1305_0708_b200/gen/flopcount.h"
+#include "../paper_1305_0708_b200/csrc/hg_couplings.h"
+#include "../paper_1305_0708_b200/csrc/hg_host_setup.h"
+#include "../paper_1305_0708_b200/csrc/generated/hg_proc_1.cuh"
+#include "../paper_1305_0708_b200/csrc/generated/hg_proc_2.cuh"
+#include "../paper_1305_0708_b200/csrc/generated/hg_proc_3.cuh"
+#include "../paper_1305_0708_b200/csrc/generated/hg_proc_4.cuh"
+#include "../paper_1305_0708_b200/csrc/generated/hg_proc_5.cuh"
+#include "../paper_1305_0708_b200/csrc/generated/hg_proc_6.cuh"
+#include "../paper_1305_0708_b200/csrc/generated/hg_proc_7.cuh"
+#include "../paper_1305_0708_b200/csrc/generated/hg_proc_8.cuh"
+#include "../paper_1305_0708_b200/csrc/generated/hg_proc_9.cuh"
 
 using namespace hg;
 

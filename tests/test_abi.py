@@ -16,13 +16,15 @@ def api():
 
 
 def test_exports_every_declared_symbol(api):
-    hdr = open(os.path.join(ROOT, 'include', 'hg.h')).read()
-    hdr = re.sub(r'/\*.*?\*/', '', hdr, flags=re.S)
-    declared = set(re.findall(r'\b(hg_[a-z0-9_]+)\s*\(', hdr))
-    assert declared == set(api.SYMBOLS)
     lib = api.load()
-    for s in declared:
-        assert hasattr(lib, s), s
+    for header, symbols in (('hg.h', api.SYMBOLS), ('hg_bench.h', api.BENCH_SYMBOLS)):
+        hdr = open(os.path.join(ROOT, 'include', header)).read()
+        hdr = re.sub(r'/\*.*?\*/', '', hdr, flags=re.S)
+        declared = set(re.findall(r'\b(hg_[a-z0-9_]+)\s*\(', hdr))
+        assert declared == set(symbols), header
+        for s in declared:
+            assert hasattr(lib, s), s
+    assert sorted(os.listdir(os.path.join(ROOT, 'include'))) == ['hg.h', 'hg_bench.h']
 
 
 def test_process_info_matches_survey_table(api):
@@ -56,3 +58,29 @@ def test_no_cpu_fallback(api):
         pytest.skip('GPU present')
     with pytest.raises(RuntimeError):
         api.Context(0)
+
+
+def test_grid_refine_matches_oracle(api):
+    """hg_grid_refine (host C++) against oracle.vegas.refine on random histograms, peaked ones, and empty rows."""
+    import numpy as np
+    import torch
+    from oracle import vegas
+    rng = np.random.default_rng(3)
+    for nb in (2, 16, 50, 64):
+        ndim = 5
+        grid = np.sort(np.concatenate([np.zeros((ndim, 1)), rng.uniform(0, 1, (ndim, nb - 1)), np.ones((ndim, 1))], 1), 1)
+        hist = rng.uniform(0, 1, (ndim, nb)) ** 8
+        hist[1] = 0.0                      # nothing accumulated: row unchanged
+        hist[2, : nb // 2] = 0.0           # empty bins
+        hist[3] = 0.0
+        hist[3, nb // 3] = 7.0             # everything in one bin
+        for alpha in (1.5, 1.0, 0.3):
+            want = vegas.refine(grid, hist, alpha)
+            got = torch.from_numpy(grid.copy())
+            api.hg_grid_refine(torch.from_numpy(hist.copy()), alpha, got)
+            got = got.numpy()
+            assert np.array_equal(got[1], grid[1])
+            assert np.allclose(got, want, rtol=0, atol=1e-14), (nb, alpha, np.abs(got - want).max())
+            assert np.all(np.diff(got, axis=1) > 0) and np.all(got[:, 0] == 0) and np.all(got[:, -1] == 1)
+    with pytest.raises(api.HgError):
+        api.hg_grid_refine(torch.zeros((2, 100), dtype=torch.float64), 1.5, torch.zeros((2, 101), dtype=torch.float64))

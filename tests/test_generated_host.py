@@ -15,7 +15,7 @@ from oracle import processes as opr
 from oracle import sm as osm
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
-SRC = os.path.join(ROOT, 'paper_1305_0708_b200', 'gen', 'hostcheck.cpp')
+SRC = os.path.join(ROOT, 'tests', 'hostcheck.cpp')
 N = {1: 64, 2: 48, 3: 24, 4: 4, 5: 6, 6: 64, 7: 48, 8: 48, 9: 3}
 
 
