@@ -32,16 +32,32 @@ if ROOT not in sys.path:
 
 METRIC = 'helicity+colour-summed |M|^2 events/s on 1 B200; % of FP64/FP32 peak'
 UNIT = 'events/s'
-SQRT_S = {1: 80.0, 2: 500.0, 3: 1000.0, 4: 1500.0, 5: 2000.0, 6: 500.0, 7: 1000.0, 8: 1000.0, 9: 3000.0}
-N_EVENTS = {1: 1 << 16, 2: 1 << 20, 3: 1 << 22, 4: 1 << 22, 5: 1 << 22, 6: 1 << 20, 7: 1 << 20, 8: 1 << 20, 9: 1 << 20}
+SQRT_S = {1: 80.0, 2: 500.0, 3: 1000.0, 4: 1500.0, 5: 2000.0, 6: 500.0, 7: 1000.0, 8: 1000.0, 9: 3000.0, 10: 1000.0,
+          11: 1000.0}
+N_EVENTS = {1: 1 << 16, 2: 1 << 20, 3: 1 << 22, 4: 1 << 22, 5: 1 << 22, 6: 1 << 20, 7: 1 << 20, 8: 1 << 20, 9: 1 << 20,
+            10: 1 << 20, 11: 1 << 20}
 NAMES = {1: 'u d~ -> e+ ve', 2: 'u u~ -> e+ e- g', 3: 'u d~ -> e+ ve g g',
          4: 'g g -> t t~ g -> b e+ ve b~ mu- vm~ g', 5: 'u d~ -> e+ ve g g g',
          6: 'u d~ -> e+ ve h', 7: 'u u~ -> e+ e- h h', 8: 'g g -> t t~ h',   # 6-8: Higgs-sector (NEXT-1)
-         9: 'u d~ -> e+ ve g g g g'}                                          # W + 4 jets (NEXT-4)
+         9: 'u d~ -> e+ ve g g g g',                                          # W + 4 jets (NEXT-4)
+         10: 'u d -> h u d', 11: 'u d -> h h u d'}                            # weak-boson fusion (NEXT-1)
 SEED = 13050708
-# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel, from the ncu --set full captures
-# summarised in profiles/ (r01_ncu_full_me_acc_cfg5_f64.txt: 247.76 MB + 4.13 MB; r01_ncu_full_me_acc_cfg4_f64.txt: 315.32 MB + 4.00 MB)
-TRAFFIC = {'cfg5_f64': 251886592, 'cfg4_f64': 319316480}
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel come from the ncu --set full
+# captures summarised in profiles/: profiles/dram_traffic.csv lists (kernel, config, dtype, events per launch, bytes
+# read, bytes written, source file); a run whose dominant-kernel launch matches no row reports traffic = null.
+def dram_traffic(kernel, cfg, dtype, events_per_launch):
+    path = os.path.join(ROOT, 'profiles', 'dram_traffic.csv')
+    try:
+        with open(path) as f:
+            rows = [ln.strip().split(',') for ln in f if ln.strip() and not ln.startswith('#')]
+    except OSError:
+        return None, 'profiles/dram_traffic.csv not found'
+    for r in rows[1:]:
+        if r[0] == kernel and int(r[1]) == cfg and r[2] == dtype and int(r[3]) == events_per_launch:
+            return int(r[4]) + int(r[5]), r[6]
+    return None, 'no ncu capture of %s for config %d %s at %d events per launch' % (kernel, cfg, dtype, events_per_launch)
+
+
 # nominal non-tensor peaks of B200: 148 SMs x 4 SMSP x 16 lanes x 2 flop x 1.965 GHz for
 # FP64 (one DFMA warp instruction per SMSP every 2 cycles) and twice that for FP32
 PEAK_NOMINAL_TFLOPS = {'f64': 148 * 64 * 2 * 1.965e9 / 1e12, 'f32': 148 * 128 * 2 * 1.965e9 / 1e12}
@@ -101,7 +117,7 @@ class ClockSampler:
 
 
 # ------------------------------------------------------------------------------------------ oracle timing
-ORACLE_SAMPLE = {1: 65536, 2: 8192, 3: 2048, 4: 48, 5: 48, 6: 8192, 7: 4096, 8: 1024, 9: 4}   # events per oracle step (about 1-3 s each)
+ORACLE_SAMPLE = {1: 65536, 2: 8192, 3: 2048, 4: 48, 5: 48, 6: 8192, 7: 4096, 8: 1024, 9: 4, 10: 8192, 11: 2048}   # events per oracle step (about 1-3 s each)
 
 
 def oracle_step(cfg, first, n, all_cores):
@@ -211,6 +227,60 @@ def measure_config(torch, api, ctx, cfg, prec, n, reps, peaks):
     return res
 
 
+def _sig(acc):
+    s = acc[0] / acc[2]
+    return s, (max(acc[1] / acc[2] - s * s, 0.0) / max(acc[2] - 1.0, 1.0)) ** 0.5
+
+
+def measure_paper_phase_space(torch, api, ctx, cfg, n, reps):
+    """the step in the paper's own phase space (hadronic sqrt(s) = 14 TeV, toy parton
+    densities, A23), flat and after a BASES-style grid optimisation (5 iterations of n points, A22):
+    events/s, pass fraction and relative Monte-Carlo error per step, beside flat RAMBO at fixed s_hat."""
+    import numpy as np
+    rs_had, nb, alpha, iters = 14000.0, 50, 1.0, 5
+    nd = api.hg_process_info(cfg)['n_draws']
+    prec = api.HG_F64
+    out = {}
+
+    def timed(fn):
+        for _ in range(2):
+            fn()
+        return statistics.median(_events_ms(torch, fn, reps))
+
+    acc = ctx.hg_integrate_step(cfg, prec, SEED, 0, n, SQRT_S[cfg])
+    s, e = _sig(acc)
+    out['rambo_fixed_shat'] = {'pass_fraction': acc[3] / acc[2], 'rel_error': e / s, 'sigma_pb': s}
+    try:
+        ctx.hg_set_hadronic(api.hg_default_hadronic(cfg))
+        acc = ctx.hg_integrate_step(cfg, prec, SEED, 0, n, rs_had)
+        ms = timed(lambda: ctx.hg_integrate_step(cfg, prec, SEED, 0, n, rs_had))
+        s, e = _sig(acc)
+        out['paper_flat'] = {'ms': ms, 'events_per_s': n / (ms * 1e-3), 'pass_fraction': acc[3] / acc[2],
+                             'rel_error': e / s, 'sigma_pb': s}
+        grid = torch.from_numpy(np.tile(np.linspace(0.0, 1.0, nb + 1), (nd, 1))).contiguous()
+        t_opt = []
+        for it in range(iters):
+            d_grid = grid.cuda()
+            d_hist = torch.zeros((nd, nb), dtype=torch.float64, device='cuda')
+            ctx.hg_set_grid(d_grid, d_hist)
+            t_opt += _events_ms(torch, lambda: ctx.hg_integrate_step(cfg, prec, SEED, (it + 1) * n, n, rs_had), 1)
+            api.hg_grid_refine(d_hist.cpu(), alpha, grid)
+        d_grid = grid.cuda()
+        ctx.hg_set_grid(d_grid, None)
+        acc = ctx.hg_integrate_step(cfg, prec, SEED, (iters + 2) * n, n, rs_had)
+        ms = timed(lambda: ctx.hg_integrate_step(cfg, prec, SEED, (iters + 2) * n, n, rs_had))
+        s, e = _sig(acc)
+        out['paper_adapted'] = {'ms': ms, 'events_per_s': n / (ms * 1e-3), 'pass_fraction': acc[3] / acc[2],
+                                'rel_error': e / s, 'sigma_pb': s, 'grid_optimisation_ms_per_iteration':
+                                statistics.median(t_opt), 'iterations': iters, 'bins': nb, 'alpha': alpha}
+        out['error_reduction_by_grid'] = out['paper_flat']['rel_error'] / out['paper_adapted']['rel_error']
+    finally:
+        ctx.hg_set_grid(None)
+        ctx.hg_set_hadronic(None)
+    out['n'] = n
+    return out
+
+
 def run_gpu(args):
     import torch
     import torch.distributed as dist
@@ -306,12 +376,13 @@ def run_gpu(args):
     me_ms_step = me_ms / args.steps                      # all launches of the dominant kernel in one step
     flops_kernel = info['flops_f64'] * n_pass + (0.0 if staged else info['flops_ps'] * n)
     achieved = flops_kernel / (me_ms_step * 1e-3) / 1e12
-    traffic = TRAFFIC.get('cfg%d_%s' % (cfg, pname))
     tname = 'double' if pname == 'f64' else 'float'
+    kname = 'me_acc_kernel' if staged else 'integrate_kernel'
+    traffic, traffic_src = dram_traffic(kname, cfg, pname, min(n, 1 << 20) if staged else n)
     roofline = {'bound': 'alu',
                 'kernel': ('me_acc_kernel<P%d,%s>' if staged else 'integrate_kernel<P%d,%s>') % (cfg, tname),
                 'achieved': achieved, 'peak': PEAK_NOMINAL_TFLOPS[pname], 'unit': 'TFLOP/s',
-                'frac': achieved / PEAK_NOMINAL_TFLOPS[pname], 'traffic': traffic,
+                'frac': achieved / PEAK_NOMINAL_TFLOPS[pname], 'traffic': traffic, 'traffic_source': traffic_src,
                 'peak_kind': 'nominal non-tensor %s peak (148 SM x %d lanes x 2 x 1.965 GHz, DESIGN.md); '
                              'MEASURED_PEAKS.json has no ALU figure' % (pname, 64 if pname == 'f64' else 128),
                 'peak_measured_fma_chain': peaks[pname], 'frac_of_measured_fma_chain': achieved / peaks[pname],
@@ -322,12 +393,13 @@ def run_gpu(args):
 
     per_config = {}
     if not args.no_table:
-        for c in (1, 2, 3, 4, 5, 6, 7, 8, 9):
+        for c in (1, 2, 3, 4, 5, 6, 7, 8, 9, 10, 11):
             for pr, nm in ((api.HG_F64, 'f64'), (api.HG_F32, 'f32')):
                 per_config['cfg%d_%s' % (c, nm)] = measure_config(torch, api, ctx, c, pr, N_EVENTS[c], 7, peaks)
         per_config['cfg1_f64_4M'] = measure_config(torch, api, ctx, 1, api.HG_F64, 1 << 22, 7, peaks)
         per_config['cfg1_f32_4M'] = measure_config(torch, api, ctx, 1, api.HG_F32, 1 << 22, 7, peaks)
 
+    paper_ps = None if args.no_table else measure_paper_phase_space(torch, api, ctx, cfg, n, 5)
     cpu_base, _ = time_oracle(cfg, 4, 1)
     s = acc[0] / acc[2]
     ds = (max(acc[1] / acc[2] - s * s, 0.0) / max(acc[2] - 1.0, 1.0)) ** 0.5
@@ -343,7 +415,8 @@ def run_gpu(args):
                                  min(n, 1 << 20) * (4 * info['n_ext'] * el + 9) >> 20, n * 4 * info['n_ext'] * el >> 20),
                        'pass_fraction': acc[3] / acc[2], 'sigma_pb': s, 'sigma_err_pb': ds},
             'clocks': clocks, 'e2e': e2e, 'gpu_launches': launches, 'roofline': roofline,
-            'cpu_baseline': cpu_base, 'fma_peak_measured_tflops': peaks, 'per_config': per_config}
+            'cpu_baseline': cpu_base, 'fma_peak_measured_tflops': peaks, 'per_config': per_config,
+            'paper_phase_space': paper_ps}
     print(json.dumps(line))
     ctx.close()
     if world > 1:
@@ -355,7 +428,7 @@ def main():
     ap.add_argument('--gpus', type=int, default=1)
     ap.add_argument('--steps', type=int, default=20)
     ap.add_argument('--warmup', type=int, default=3)
-    ap.add_argument('--config', type=int, default=5, choices=[1, 2, 3, 4, 5, 6, 7, 8, 9])
+    ap.add_argument('--config', type=int, default=5, choices=[1, 2, 3, 4, 5, 6, 7, 8, 9, 10, 11])
     ap.add_argument('--dtype', default='f64', choices=['f64', 'f32'])
     ap.add_argument('--events', type=int, default=0, help='events per GPU per step (default: BASELINE.json size)')
     ap.add_argument('--impl', default='graft', choices=['graft', 'reference'])

@@ -66,9 +66,15 @@ enum hg_process {
   HG_GG_TTXH = 8,
   /* next size up: u d~ -> e+ ve g g g g, 8 legs, 428 Feynman diagrams / 516
    * colour-split amplitudes, 24 colour flows, 16 of 256 helicity combinations non-zero; cuts as config 5 */
-  HG_UDX_EPVEGGGG = 9
+  HG_UDX_EPVEGGGG = 9,
+  /* weak-boson fusion (Eq. 21a, 22a): two quark lines, W W and Z Z
+   * fusion with their interference (two colour flows, relative Fermi sign); no cuts; massive RAMBO.
+   *   HG_UD_HUD    u d -> h u d      (5 legs)  W W H, Z Z H
+   *   HG_UD_HHUD   u d -> h h u d    (6 legs)  + W W H H, Z Z H H, H H H */
+  HG_UD_HUD = 10,
+  HG_UD_HHUD = 11
 };
-#define HG_N_PROCESS 9
+#define HG_N_PROCESS 11
 #define HG_MAX_EXT 9
 
 /* Standard Model inputs (paper's own: PAPER.md:1075; the configs override them).
@@ -174,6 +180,28 @@ int hg_accumulate(hg_ctx* ctx, int precision, int64_t n, const void* d_me2, cons
  * Synchronises the stream; acc (HOST, overwritten) = (sum w, sum w^2, n, n_pass).  sigma = acc[0]/acc[2]. */
 int hg_integrate_step(hg_ctx* ctx, int process, int precision, uint64_t seed, uint64_t first_event,
                       int64_t n, double sqrt_s_hat, double acc[4], void* cuda_stream);
+
+/* The paper's own phase-space parameterisation for hadron collisions (Section 3 and Appendix A, PAPER.md:358-393,
+ * 1110-1194; reading A23): integration variables y_i, ln(pT_i^2 + m_i^2), phi_i and the Breit-Wigner
+ * mapped resonance masses, with the parton momentum fractions x_a, x_b following from momentum conservation
+ * (Eq. 24, A.9) and a null weight for x >= 1 (A.10).  Every jet's pT and rapidity cut is built into the ranges
+ * (|y_jet| < eta_jet_max of the cuts, or 5 when that cut is off; pT_jet from pt_jet_min, or 1 GeV, to sqrt(s)/2);
+ * the resonance (W, Z, or the second top of config 4) takes the recoil and has |y| < y_res_max.  CTEQ6L1 is not
+ * available: the parton density of beam parton i is the toy  f(x) = pdf_norm[i] x^-pdf_a[i] (1 - x)^pdf_b[i].
+ *
+ * After hg_set_hadronic(ctx, h) with h != NULL, hg_gen_phase_space and hg_integrate_step take their sqrt_s_hat
+ * argument as the HADRONIC sqrt(s); momenta are in the lab frame (incoming partons x_a, x_b along +-z); d_wps is
+ * dSigma-weight * f_a f_b * s / s_hat, so that w = pass * me2 * wps * (hbar c)^2 / (2 s) as before; a point with
+ * x_a >= 1 or x_b >= 1 has wps = 0 and pass = 0.  Implemented for HG_UDX_EPVE, HG_UUX_EPEMG, HG_UDX_EPVEGG,
+ * HG_GG_TTXG_DILEP, HG_UDX_EPVEGGG, HG_UDX_EPVEGGGG (HG_EINVAL otherwise).  h == NULL returns to RAMBO at fixed s_hat.
+ * hg_default_hadronic: valence-like (2.2, 0.5, 3) and sea-like (0.2, 1.2, 7) quark densities (gluon (3, 1.2, 5) for
+ * config 4), y_res_max = 4. */
+typedef struct {
+  double y_res_max;
+  double pdf_norm[2], pdf_a[2], pdf_b[2];
+} hg_hadronic;
+int hg_default_hadronic(int process, hg_hadronic* out);
+int hg_set_hadronic(hg_ctx* ctx, const hg_hadronic* h);
 
 /* Adaptive sampling grid of the integration (role of the BASES grid: "a grid-optimisation step followed by an
  * integration step"; the algorithm is the published VEGAS one, reading A22).

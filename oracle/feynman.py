@@ -463,16 +463,55 @@ def root_amplitudes(root, hel, kin, memo=None):
     moms = [kin.momentum(c.legs) for c in chs]
     fields = [c.field for c in chs]
     wl = kin.wf[(last.leg, hel[last.leg])]
+    sign = fermion_sign(root)
     out = []
     for combo in itertools.product(*lists):
         for cur in _vertex_currents(v, fields, list(combo), moms):
             if spin(last.field) == 'S':
-                out.append(cur * wl)
+                out.append(sign * cur * wl)
             elif spin(last.field) == 'V':
-                out.append(D.mdot(cur, wl))
+                out.append(sign * D.mdot(cur, wl))
             else:
-                out.append(np.einsum('na,na->n', cur, wl))
+                out.append(sign * np.einsum('na,na->n', cur, wl))
     return out
+
+
+def fermion_lines(root):
+    """The fermion lines of a diagram as (row leg, column leg) pairs: the external leg at the END of the fermion
+    arrow (its wavefunction is a row spinor, psibar) and the one at its START (a column spinor)."""
+    lines = []
+
+    def walk(tree):
+        """Returns the open end ('row' | 'col', leg) of the fermion line that leaves `tree` towards its parent."""
+        if isinstance(tree, Leaf):
+            if spin(tree.field) != 'F':
+                return None
+            return ('row' if is_row(tree.field) else 'col', tree.leg)
+        ends = [e for e in (walk(ch) for ch in tree.children) if e is not None]
+        if len(ends) == 2:                       # both ends meet at this vertex: the line is complete
+            (k1, l1), (k2, l2) = ends
+            assert {k1, k2} == {'row', 'col'}
+            lines.append((l1, l2) if k1 == 'row' else (l2, l1))
+            return None
+        assert len(ends) <= 1
+        return ends[0] if ends else None
+
+    assert walk(root) is None
+    return sorted(lines)
+
+
+def fermion_sign(root):
+    """Relative sign of a diagram from Fermi statistics: the diagram is a product of spinor chains
+    (psibar_r1 ... psi_c1)(psibar_r2 ... psi_c2)...; its sign is the parity of the permutation that brings
+    (r1, c1, r2, c2, ...) to the reference order of the external fermion legs (increasing leg number).  Diagrams
+    with a single fermion line all have the same sign."""
+    seq = [l for pair in fermion_lines(root) for l in pair]
+    sign = 1
+    for i in range(len(seq)):
+        for j in range(i + 1, len(seq)):
+            if seq[i] > seq[j]:
+                sign = -sign
+    return sign
 
 
 def root_colour(root):

@@ -116,11 +116,12 @@ def two_body(P, M2, m1sq, m2sq, uc, uf):
     return boost(p1, P, M, m1sq), boost(p2, P, M, m2sq), pst / (4.0 * math.pi * M)
 
 
-N_FINAL = {1: 2, 2: 3, 3: 4, 5: 5, 6: 3, 7: 4, 8: 3, 9: 6}
-N_DRAWS = {1: 8, 2: 12, 3: 16, 4: 24, 5: 20, 6: 12, 7: 16, 8: 12, 9: 24}
-N_EXT = {1: 4, 2: 5, 3: 6, 4: 9, 5: 7, 6: 5, 7: 6, 8: 5, 9: 8}
+N_FINAL = {1: 2, 2: 3, 3: 4, 5: 5, 6: 3, 7: 4, 8: 3, 9: 6, 10: 3, 11: 4}
+N_DRAWS = {1: 8, 2: 12, 3: 16, 4: 24, 5: 20, 6: 12, 7: 16, 8: 12, 9: 24, 10: 12, 11: 16}
+N_EXT = {1: 4, 2: 5, 3: 6, 4: 9, 5: 7, 6: 5, 7: 6, 8: 5, 9: 8, 10: 5, 11: 6}
 # masses of the final-state legs of the Higgs-sector processes (parameter names; None = massless)
-FINAL_MASSES = {6: (None, None, 'mh'), 7: (None, None, 'mh', 'mh'), 8: ('mt', 'mt', 'mh')}
+FINAL_MASSES = {6: (None, None, 'mh'), 7: (None, None, 'mh', 'mh'), 8: ('mt', 'mt', 'mh'), 10: ('mh', None, None),
+                11: ('mh', 'mh', None, None)}
 
 
 def generate(cfg, seed, first_event, n, rs, par, grid=None, with_bins=False):
@@ -177,8 +178,8 @@ def default_cuts(cfg):
             4: (20.0, 2.5, 0.0, 0.0), 5: (20.0, 2.5, 0.0, 0.4), 9: (20.0, 2.5, 0.0, 0.4)}.get(cfg, (0.0, 0.0, 0.0, 0.0))
 
 
-JETS = {1: [], 2: [4], 3: [4, 5], 4: [8], 5: [4, 5, 6], 6: [], 7: [], 8: [], 9: [4, 5, 6, 7]}  # gluon legs
-CHARGED_LEPTONS = {1: [2], 2: [2, 3], 3: [2], 4: [3, 6], 5: [2], 6: [2], 7: [2, 3], 8: [], 9: [2]}
+JETS = {1: [], 2: [4], 3: [4, 5], 4: [8], 5: [4, 5, 6], 6: [], 7: [], 8: [], 9: [4, 5, 6, 7], 10: [], 11: []}  # gluon legs
+CHARGED_LEPTONS = {1: [2], 2: [2, 3], 3: [2], 4: [3, 6], 5: [2], 6: [2], 7: [2, 3], 8: [], 9: [2], 10: [], 11: []}
 
 
 def pt(p):

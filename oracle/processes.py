@@ -163,9 +163,17 @@ def config(i):
     if i == 9:   # next size up: W + 4 jets, 428 diagrams, 516 colour-split terms
         return Process('udx_epvegggg', ['u', 'd~'], ['e+', 've', 'g', 'g', 'g', 'g'],
                        ['udw', 'enw', 'uug', 'ddg', 'ggg', 'gggg'])
+    # weak-boson fusion: two quark lines (Eq. 21a, 22a)
+    if i == 10:
+        return Process('ud_hud', ['u', 'd'], ['h', 'u', 'd'], ['uuz', 'ddz', 'udw', 'zzh', 'wwh'])
+    if i == 11:
+        return Process('ud_hhud', ['u', 'd'], ['h', 'h', 'u', 'd'],
+                       ['uuz', 'ddz', 'udw', 'zzh', 'wwh', 'zzhh', 'wwhh', 'hhh'])
     raise ValueError(i)
 
 
 # sqrt(s_hat) [GeV] and number of events of each config (BASELINE.json)
-SQRT_S = {1: 80.0, 2: 500.0, 3: 1000.0, 4: 1500.0, 5: 2000.0, 6: 500.0, 7: 1000.0, 8: 1000.0, 9: 3000.0}
-N_EVENTS = {1: 1 << 16, 2: 1 << 20, 3: 1 << 22, 4: 1 << 22, 5: 1 << 22, 6: 1 << 20, 7: 1 << 20, 8: 1 << 20, 9: 1 << 20}
+SQRT_S = {1: 80.0, 2: 500.0, 3: 1000.0, 4: 1500.0, 5: 2000.0, 6: 500.0, 7: 1000.0, 8: 1000.0, 9: 3000.0, 10: 1000.0,
+          11: 1000.0}
+N_EVENTS = {1: 1 << 16, 2: 1 << 20, 3: 1 << 22, 4: 1 << 22, 5: 1 << 22, 6: 1 << 20, 7: 1 << 20, 8: 1 << 20, 9: 1 << 20,
+            10: 1 << 20, 11: 1 << 20}

@@ -11,13 +11,13 @@ import torch
 
 HG_F64, HG_F32 = 0, 1
 HG_UDX_EPVE, HG_UUX_EPEMG, HG_UDX_EPVEGG, HG_GG_TTXG_DILEP, HG_UDX_EPVEGGG = 1, 2, 3, 4, 5
-PROCESSES = (1, 2, 3, 4, 5, 6, 7, 8, 9)
+PROCESSES = (1, 2, 3, 4, 5, 6, 7, 8, 9, 10, 11)
 HG_OK, HG_EINVAL, HG_ENOPROC, HG_ECUDA, HG_ENOTSET = 0, -1, -2, -3, -4
 
 # symbols include/hg.h declares (checked by tests/test_abi.py)
 SYMBOLS = ('hg_create', 'hg_destroy', 'hg_last_error', 'hg_default_params', 'hg_default_cuts', 'hg_process_info',
            'hg_set_params', 'hg_gen_phase_space', 'hg_matrix_element', 'hg_matrix_element_host', 'hg_accumulate',
-           'hg_integrate_step', 'hg_set_grid', 'hg_grid_refine')
+           'hg_integrate_step', 'hg_set_grid', 'hg_grid_refine', 'hg_default_hadronic', 'hg_set_hadronic')
 HG_GRID_MAX_BINS = 64
 # measurement helpers of include/hg_bench.h (bench.py only)
 BENCH_SYMBOLS = ('hg_set_profiling', 'hg_last_step_info', 'hg_measure_fma_peak')
@@ -30,6 +30,11 @@ class hg_params(C.Structure):
 
 class hg_cuts(C.Structure):
     _fields_ = [(n, C.c_double) for n in ('pt_jet_min', 'eta_jet_max', 'eta_lep_max', 'dr_jj_min')]
+
+
+class hg_hadronic(C.Structure):
+    _fields_ = [('y_res_max', C.c_double), ('pdf_norm', C.c_double * 2), ('pdf_a', C.c_double * 2),
+                ('pdf_b', C.c_double * 2)]
 
 
 class hg_process_info_t(C.Structure):
@@ -76,6 +81,8 @@ def load():
     L.hg_matrix_element_host.argtypes = [vp, i32, i32, i64, vp, vp, vp]
     L.hg_accumulate.argtypes = [vp, i32, i64, vp, vp, vp, dbl, C.POINTER(dbl), vp]
     L.hg_integrate_step.argtypes = [vp, i32, i32, u64, u64, i64, dbl, C.POINTER(dbl), vp]
+    L.hg_default_hadronic.argtypes = [i32, C.POINTER(hg_hadronic)]
+    L.hg_set_hadronic.argtypes = [vp, C.POINTER(hg_hadronic)]
     L.hg_set_grid.argtypes = [vp, vp, i32, vp]
     L.hg_grid_refine.argtypes = [i32, i32, vp, dbl, vp]
     L.hg_measure_fma_peak.argtypes = [vp, i32, C.POINTER(dbl), vp]
@@ -97,6 +104,14 @@ def hg_default_cuts(process):
     if rc != HG_OK:
         raise HgError(rc, 'unknown process id')
     return c
+
+
+def hg_default_hadronic(process):
+    h = hg_hadronic()
+    rc = load().hg_default_hadronic(process, C.byref(h))
+    if rc != HG_OK:
+        raise HgError(rc, 'unknown process id')
+    return h
 
 
 def hg_process_info(process):
@@ -233,6 +248,10 @@ class Context:
         self._check(self._L.hg_integrate_step(self._h, process, precision, seed, first_event, n, sqrt_s_hat, acc,
                                               _stream(stream)))
         return tuple(acc)
+
+    def hg_set_hadronic(self, had):
+        """had: hg_hadronic (the paper's hadronic phase space with toy parton densities) or None (RAMBO at fixed s_hat)."""
+        self._check(self._L.hg_set_hadronic(self._h, C.byref(had) if had is not None else None))
 
     def hg_set_grid(self, grid, hist=None):
         """grid: CUDA float64 tensor [n_draws, n_bins + 1] (kept alive by the context wrapper) or None for flat

@@ -25,6 +25,8 @@ static const ProcVTable* vtable(int process) {
     case HG_UUX_EPEMHH: return &hg_proc_7;
     case HG_GG_TTXH: return &hg_proc_8;
     case HG_UDX_EPVEGGGG: return &hg_proc_9;
+    case HG_UD_HUD: return &hg_proc_10;
+    case HG_UD_HHUD: return &hg_proc_11;
   }
   return nullptr;
 }
@@ -48,6 +50,8 @@ struct hg_ctx {
   size_t stage_bytes = 0;
   void* d_scratch = nullptr;     // phase-space points of one chunk of hg_integrate_step (staged processes)
   size_t scratch_bytes = 0;
+  bool hadronic = false;           // hg_set_hadronic
+  hg_hadronic had;
   const double* d_grid = nullptr;  // hg_set_grid: caller-owned [n_draws][grid_nb + 1]
   int grid_nb = 0;
   double* d_hist = nullptr;        // caller-owned [n_draws][grid_nb], or NULL
@@ -249,6 +253,21 @@ struct DeviceGuard {
   DeviceGuard hg_guard((ctx)->device);                                      \
   if (hg_guard.err != cudaSuccess) return fail_cuda((ctx), hg_guard.err, who ": cudaSetDevice")
 
+// sampling state of the context -> per-call constants
+static void apply_sampling(const hg_ctx* ctx, PsConst& k) {
+  k.grid = ctx->d_grid;
+  k.nb = ctx->grid_nb;
+  if (ctx->hadronic) {
+    k.had = 1;
+    k.y_res_max = ctx->had.y_res_max;
+    for (int i = 0; i < 2; ++i) {
+      k.pdf_norm[i] = ctx->had.pdf_norm[i];
+      k.pdf_a[i] = ctx->had.pdf_a[i];
+      k.pdf_b[i] = ctx->had.pdf_b[i];
+    }
+  }
+}
+
 static bool misaligned(const void* p, size_t al) { return ((uintptr_t)p % al) != 0; }
 
 static bool finite_pos(double x) { return isfinite(x) && x > 0.0; }
@@ -385,6 +404,13 @@ static const ProcVTable* check(hg_ctx* ctx, int process, int precision, int64_t 
 
 static int check_rs(hg_ctx* ctx, const ProcVTable* vt, int process, double rs, const char* who) {
   if (!finite_pos(rs)) return fail(ctx, HG_EINVAL, (std::string(who) + ": sqrt_s_hat must be finite and > 0").c_str());
+  if (ctx->hadronic) {
+    if (!vt->has_hadronic())
+      return fail(ctx, HG_EINVAL, (std::string(who) + ": the hadronic phase space is not implemented for this process").c_str());
+    const double ptmin = ctx->cuts[process].pt_jet_min > 0 ? ctx->cuts[process].pt_jet_min : 1.0;
+    if (!(2.0 * ptmin < rs)) return fail(ctx, HG_EINVAL, (std::string(who) + ": sqrt(s) below twice the jet pT cut").c_str());
+    return HG_OK;
+  }
   if (process == HG_GG_TTXG_DILEP) {
     // the Breit-Wigner windows must always be kinematically open (reading A14): no rejection on the device
     const double mtmax = sqrt(ctx->par.mt * ctx->par.mt + ctx->par.mt * ctx->par.gt * fmin(20.0, ctx->par.mt / ctx->par.gt));
@@ -398,6 +424,8 @@ static int check_rs(hg_ctx* ctx, const ProcVTable* vt, int process, double rs, c
   if (process == HG_UDX_EPVEH) msum = ctx->par.mh;
   if (process == HG_UUX_EPEMHH) msum = 2.0 * ctx->par.mh;
   if (process == HG_GG_TTXH) msum = 2.0 * ctx->par.mt + ctx->par.mh;
+  if (process == HG_UD_HUD) msum = ctx->par.mh;
+  if (process == HG_UD_HHUD) msum = 2.0 * ctx->par.mh;
   if (!(msum < rs)) return fail(ctx, HG_EINVAL, (std::string(who) + ": sqrt_s_hat is below the threshold").c_str());
   (void)vt;
   return HG_OK;
@@ -416,8 +444,7 @@ int hg_gen_phase_space(hg_ctx* ctx, int process, int precision, uint64_t seed, u
   HG_ON_DEVICE(ctx, "hg_gen_phase_space");
   const int n_rambo = process == HG_GG_TTXG_DILEP ? 3 : vt->info.n_final;
   PsConst k = make_psconst(ctx->par, ctx->cuts[process], n_rambo, sqrt_s_hat);
-  k.grid = ctx->d_grid;
-  k.nb = ctx->grid_nb;
+  apply_sampling(ctx, k);
   cudaError_t e = vt->ps(precision, n, k, seed, first_event, d_p, d_wps, d_pass, (cudaStream_t)cuda_stream);
   if (e != cudaSuccess) return fail_cuda(ctx, e, "hg_gen_phase_space");
   return HG_OK;
@@ -557,10 +584,9 @@ int hg_integrate_step(hg_ctx* ctx, int process, int precision, uint64_t seed, ui
   cudaStream_t s = (cudaStream_t)cuda_stream;
   const int n_rambo = process == HG_GG_TTXG_DILEP ? 3 : vt->info.n_final;
   PsConst k = make_psconst(ctx->par, ctx->cuts[process], n_rambo, sqrt_s_hat);
-  k.grid = ctx->d_grid;
-  k.nb = ctx->grid_nb;
+  apply_sampling(ctx, k);
   const bool hist = ctx->d_grid && ctx->d_hist;      // grid-optimisation step: accumulate the histograms
-  const bool split = vt->split_step() || ctx->d_grid != nullptr;   // grid sampling: always the split step
+  const bool split = vt->split_step() || ctx->d_grid != nullptr || ctx->hadronic;   // grid / hadronic: split step
   const double wscale = kHbarC2Pb / (2.0 * sqrt_s_hat * sqrt_s_hat);
   int per_sm = 1;
   cudaError_t e = vt->int_blocks_per_sm(precision, split, &per_sm);
@@ -628,6 +654,26 @@ int hg_integrate_step(hg_ctx* ctx, int process, int precision, uint64_t seed, ui
     }
   }
   return rc;
+}
+
+int hg_default_hadronic(int process, hg_hadronic* out) {
+  if (!out) return HG_EINVAL;
+  return default_hadronic(process, out) ? HG_OK : HG_ENOPROC;
+}
+
+int hg_set_hadronic(hg_ctx* ctx, const hg_hadronic* h) {
+  if (!ctx) return HG_EINVAL;
+  if (!h) {
+    ctx->hadronic = false;
+    return HG_OK;
+  }
+  if (!finite_pos(h->y_res_max)) return fail(ctx, HG_EINVAL, "hg_set_hadronic: y_res_max must be finite and > 0");
+  for (int i = 0; i < 2; ++i)
+    if (!finite_nonneg(h->pdf_norm[i]) || !isfinite(h->pdf_a[i]) || !finite_nonneg(h->pdf_b[i]))
+      return fail(ctx, HG_EINVAL, "hg_set_hadronic: parton-density parameters must be finite, norm and b >= 0");
+  ctx->had = *h;
+  ctx->hadronic = true;
+  return HG_OK;
 }
 
 int hg_set_grid(hg_ctx* ctx, const double* d_grid, int n_bins, double* d_hist) {

@@ -495,6 +495,60 @@ HG_HD void close_proj(const Vc<T>& e, const Vc<T>& b, cx<T>& rb, cx<T>& ib) {
   ib = mk<T>(e.c[1].im * b.c[1].re + e.c[2].im * b.c[2].re + e.c[3].im * b.c[3].re,
              e.c[1].im * b.c[1].im + e.c[2].im * b.c[2].im + e.c[3].im * b.c[3].im);
 }
+// Closing an FFV vertex on the massless vector leg through a DRESSED spinor.  rb = sum_i x_i J_i (i = 1..3) with
+// J = ffv_current(fi, fo) and x = Re eps(+1) (PART = 0) or Im eps(+1) (PART = 1; its third component vanishes) is
+// bilinear in the two spinors:  rb = D . fi  with the row spinor D = <fo| x_i gamma^i (gL PL + gR PR), or
+// rb = fo . C  with the column spinor C.  When one of the spinors lives outside the helicity loops the generator
+// dresses it once per event (dress_row / dress_col) and every closing inside the loops is a plain spinor dot
+// product (sdot): 2 complex FMAs per chirality instead of the current + projection (gen/emit.py "closing by spinor").
+//   L part (fo slots B, fi slots A):  J_1 = -gL (r0 c1 + r1 c0), J_2 = i gL (r0 c1 - r1 c0), J_3 = gL (r1 c1 - r0 c0)
+//   R part (fo slots A, fi slots B):  J_1 =  gR (r0 c1 + r1 c0), J_2 = i gR (r1 c0 - r0 c1), J_3 = gR (r0 c0 - r1 c1)
+template <int PART, class T>
+HG_HD void dress_pair(const Vc<T>& e, T g, cx<T> s0, cx<T> s1, bool row, bool left, cx<T>& d0, cx<T>& d1) {
+  const T x1 = PART ? e.c[1].im : e.c[1].re, x2 = PART ? e.c[2].im : e.c[2].re;
+  // (x1 + i x2) and (x1 - i x2): a dressed row has the "+" one in d0, a dressed column the "-" one
+  const bool plus_first = row;
+  const cx<T> p = mk<T>(x1, plus_first ? x2 : -x2), m = mk<T>(x1, plus_first ? -x2 : x2);
+  cx<T> a = p * s1, b = m * s0;
+  if (PART == 0) {
+    const T x3 = e.c[3].re;
+    a = a + x3 * s0;
+    b = b - x3 * s1;
+  }
+  // L part: d0 = -g (x3 s0 + p s1), d1 = g (x3 s1 - m s0);  R part: the opposite sign
+  const T gs = left ? -g : g;
+  d0 = gs * a;
+  d1 = gs * b;
+}
+template <int MO, int G, int PART, class T>
+HG_HD Sp<T> dress_row(const Sp<T>& fo, const Vc<T>& e, T gL, T gR) {
+  Sp<T> d;
+  for (int i = 0; i < 4; ++i) d.c[i] = czero<T>();
+  if ((MO & SLOT_B) && (G & CPL_L)) dress_pair<PART>(e, gL, fo.c[2], fo.c[3], true, true, d.c[0], d.c[1]);
+  if ((MO & SLOT_A) && (G & CPL_R)) dress_pair<PART>(e, gR, fo.c[0], fo.c[1], true, false, d.c[2], d.c[3]);
+  return d;
+}
+template <int MI, int G, int PART, class T>
+HG_HD Sp<T> dress_col(const Sp<T>& fi, const Vc<T>& e, T gL, T gR) {
+  Sp<T> d;
+  for (int i = 0; i < 4; ++i) d.c[i] = czero<T>();
+  if ((MI & SLOT_A) && (G & CPL_L)) dress_pair<PART>(e, gL, fi.c[0], fi.c[1], false, true, d.c[2], d.c[3]);
+  if ((MI & SLOT_B) && (G & CPL_R)) dress_pair<PART>(e, gR, fi.c[2], fi.c[3], false, false, d.c[0], d.c[1]);
+  return d;
+}
+// plain (unconjugated) dot product of two spinors over the slot pairs of mask M
+template <int M, class T>
+HG_HD cx<T> sdot(const Sp<T>& a, const Sp<T>& b) {
+  cx<T> r = czero<T>();
+  if (M & SLOT_A) r = cfma(a.c[1], b.c[1], a.c[0] * b.c[0]);
+  if (M & SLOT_B) {
+    if (M & SLOT_A)
+      r = cfma(a.c[3], b.c[3], cfma(a.c[2], b.c[2], r));
+    else
+      r = cfma(a.c[3], b.c[3], a.c[2] * b.c[2]);
+  }
+  return r;
+}
 // amplitude for helicity sign s from the accumulated projections
 template <class T>
 HG_HD cx<T> close_amp(cx<T> x, cx<T> y, T s) {

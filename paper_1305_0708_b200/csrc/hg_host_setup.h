@@ -35,9 +35,26 @@ inline bool default_cuts(int process, hg_cuts* c) {
     case HG_UDX_EPVEGGGG: *c = hg_cuts{20.0, 2.5, 0.0, 0.4}; return true;
     case HG_UDX_EPVEH:
     case HG_UUX_EPEMHH:
-    case HG_GG_TTXH: *c = hg_cuts{0.0, 0.0, 0.0, 0.0}; return true;
+    case HG_GG_TTXH:
+    case HG_UD_HUD:
+    case HG_UD_HHUD: *c = hg_cuts{0.0, 0.0, 0.0, 0.0}; return true;
   }
   return false;
+}
+
+inline bool default_hadronic(int process, hg_hadronic* h) {
+  const double val[3] = {2.2, 0.5, 3.0}, sea[3] = {0.2, 1.2, 7.0}, glu[3] = {3.0, 1.2, 5.0};
+  if (process < 1 || process > HG_N_PROCESS) return false;
+  const double* a = process == HG_GG_TTXG_DILEP ? glu : val;
+  const double* b = process == HG_GG_TTXG_DILEP ? glu : sea;
+  h->y_res_max = 4.0;
+  h->pdf_norm[0] = a[0];
+  h->pdf_a[0] = a[1];
+  h->pdf_b[0] = a[2];
+  h->pdf_norm[1] = b[0];
+  h->pdf_a[1] = b[1];
+  h->pdf_b[1] = b[2];
+  return true;
 }
 
 // n_rambo = number of momenta the RAMBO stage generates (n_final, or 3 for config 4).
@@ -59,6 +76,19 @@ inline PsConst make_psconst(const hg_params& par, const hg_cuts& cuts, int n_ram
   k.dr_jj_min = cuts.dr_jj_min;
   k.grid = nullptr;
   k.nb = 0;
+  k.had = 0;
+  k.mz = par.mz;
+  k.mgz = par.mz * par.gz;
+  k.tmax_z = par.gz > 0 ? atan(fmin(20.0, par.mz / par.gz)) : 0.0;
+  k.y_jet_max = cuts.eta_jet_max > 0 ? cuts.eta_jet_max : 5.0;
+  const double ptmin = cuts.pt_jet_min > 0 ? cuts.pt_jet_min : 1.0;
+  k.lnpt_lo = log(ptmin * ptmin);
+  k.lnpt_hi = log(0.25 * rs * rs);
+  k.y_res_max = 0.0;
+  for (int i = 0; i < 2; ++i) {
+    k.pdf_norm[i] = 1.0;
+    k.pdf_a[i] = k.pdf_b[i] = 0.0;
+  }
   return k;
 }
 

@@ -50,8 +50,10 @@ struct ProcVTable {
   // bytes of the chunk buffer of the split step for `chunk` events; grid: with the histogram sections
   size_t (*scratch_bytes)(int prec, int64_t chunk, bool grid);
   bool (*split_step)();
+  bool (*has_hadronic)();   // the paper's hadronic phase space is implemented for this process
 };
 
-extern const ProcVTable hg_proc_1, hg_proc_2, hg_proc_3, hg_proc_4, hg_proc_5, hg_proc_6, hg_proc_7, hg_proc_8, hg_proc_9;
+extern const ProcVTable hg_proc_1, hg_proc_2, hg_proc_3, hg_proc_4, hg_proc_5, hg_proc_6, hg_proc_7, hg_proc_8, hg_proc_9,
+    hg_proc_10, hg_proc_11;
 
 }  // namespace hg

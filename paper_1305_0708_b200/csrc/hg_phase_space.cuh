@@ -44,6 +44,12 @@ struct PsConst {
   // [0, 1], or NULL for flat sampling
   const double* grid;
   int nb;
+  // the paper's hadronic phase space (hg_set_hadronic, reading A23; Eq. 24-28, App. A): rs is then the HADRONIC
+  // sqrt(s); ranges of the integration variables and the toy parton densities f(x) = N x^-a (1 - x)^b of the beams
+  int had;                 // 0: RAMBO at fixed s_hat; 1: hadronic
+  double mz, mgz, tmax_z;
+  double y_jet_max, lnpt_lo, lnpt_hi, y_res_max;
+  double pdf_norm[2], pdf_a[2], pdf_b[2];
 };
 
 // Grid-optimised sampling (role of the BASES grid; VEGAS algorithm, reading A22):
@@ -270,6 +276,134 @@ HG_HD double gen_ttxg_dilep(const PsConst& k, uint64_t seed, uint64_t event, uin
   w *= two_body(wm, swm, 0.0, 0.0, u[22], u[23], p[6], p[7]);
   p[8] = q[2];
   return w;
+}
+
+
+// ---------------------------------------------------------------- the paper's hadronic phase space (reading A23)
+// Eq. 24 / A.7 for n particles: y[i] (i < n), ln(pT^2 + m^2) and phi (i < n - 1) given;
+// particle n - 1 takes the recoil (A.9a).  Writes the momenta, x_a, x_b (A.9b, c) and returns
+// 1 / (2 s (4 pi)^(2n-3)) prod_{i<n-1} (pT_i^2 + m_i^2)  (Eq. 28 / A.11: dpT^2 = (pT^2 + m^2) d ln(pT^2 + m^2)).
+template <int N>
+HG_HD double generalised_ps(const double* y, const double* lnpt2m, const double* phi, const double* m2, double rs,
+                            Mom<double>* k, double& xa, double& xb) {
+  double w = 1.0 / (2.0 * rs * rs);
+  if (N == 1) w *= 2.0 * HG_TWO_PI;   // (4 pi)^-(2N-3) with 2N - 3 = -1
+#pragma unroll
+  for (int i = 0; i < 2 * N - 3; ++i) w *= 1.0 / (2.0 * HG_TWO_PI);
+  double px = 0.0, py = 0.0, sp = 0.0, sm = 0.0;
+#pragma unroll
+  for (int i = 0; i < N; ++i) {
+    double kx, ky, mt2;
+    if (i < N - 1) {
+      mt2 = exp(lnpt2m[i]);
+      const double pt = sqrt(fmax(mt2 - m2[i], 0.0));
+      double sf, cf;
+      hsincos2pi(phi[i], sf, cf);           // phi[i] holds the uniform: angle = 2 pi u
+      kx = pt * cf;
+      ky = pt * sf;
+      px += kx;
+      py += ky;
+      w *= mt2;
+    } else {
+      kx = -px;
+      ky = -py;
+      mt2 = m2[i] + kx * kx + ky * ky;
+    }
+    const double mt = sqrt(mt2);
+    k[i] = mkmom<double>(mt * cosh(y[i]), kx, ky, mt * sinh(y[i]));
+    sp += k[i].e + k[i].z;
+    sm += k[i].e - k[i].z;
+  }
+  xa = sp / rs;
+  xb = sm / rs;
+  return w;
+}
+
+HG_HD double toy_pdf(double x, double norm, double a, double b) { return norm * pow(x, -a) * pow(1.0 - x, b); }
+
+// incoming legs from x_a, x_b; parton densities and s / s_hat; a point with x >= 1 gets a null weight (A.10)
+HG_HD double had_finish(const PsConst& k, double w, double xa, double xb, Mom<double>* p) {
+  const double ea = 0.5 * k.rs * xa, eb = 0.5 * k.rs * xb;
+  p[0] = mkmom<double>(ea, 0.0, 0.0, ea);
+  p[1] = mkmom<double>(eb, 0.0, 0.0, -eb);
+  if (!(xa < 1.0 && xb < 1.0)) return 0.0;
+  const double fa = toy_pdf(xa, k.pdf_norm[0], k.pdf_a[0], k.pdf_b[0]);
+  const double fb = toy_pdf(xb, k.pdf_norm[1], k.pdf_a[1], k.pdf_b[1]);
+  return w * fa * fb / (xa * xb);
+}
+
+// W/Z + NJ jets (configs 1, 2, 3, 5, 9): draws 0: s_R; 1+3j, 2+3j, 3+3j: y, ln pT^2, phi of jet j; 1+3NJ: y_R;
+// 2+3NJ, 3+3NJ: decay angles of R -> l l'.  Legs: 2, 3 = the leptons, 4.. = the jets.
+template <int NJ, int NDRAW, bool GRID>
+HG_HD double gen_had_vjets(const PsConst& k, uint64_t seed, uint64_t event, uint32_t pid, double mres, double mgres,
+                           double tmax, Mom<double>* p, uint8_t* bins) {
+  double u[NDRAW];
+  draw_uniforms<NDRAW>(seed, event, pid, u);
+  double jac = 1.0;
+  if constexpr (GRID) jac = grid_map<NDRAW>(k, u, bins);
+  double sR;
+  double w = jac * bw_mass(u[0], mres, mgres, tmax, sR);
+  constexpr int N = NJ + 1;
+  double y[N], lnpt[N], phi[N], m2[N];
+#pragma unroll
+  for (int j = 0; j < NJ; ++j) {
+    y[j] = k.y_jet_max * (2.0 * u[1 + 3 * j] - 1.0);
+    lnpt[j] = k.lnpt_lo + (k.lnpt_hi - k.lnpt_lo) * u[2 + 3 * j];
+    phi[j] = u[3 + 3 * j];
+    m2[j] = 0.0;
+    w *= (2.0 * k.y_jet_max) * (k.lnpt_hi - k.lnpt_lo);
+  }
+  y[NJ] = k.y_res_max * (2.0 * u[1 + 3 * NJ] - 1.0);
+  w *= 2.0 * k.y_res_max;
+  m2[NJ] = sR;
+  lnpt[NJ] = phi[NJ] = 0.0;
+  Mom<double> q[N];
+  double xa, xb;
+  w *= generalised_ps<N>(y, lnpt, phi, m2, k.rs, q, xa, xb);
+  w *= two_body(q[NJ], sR, 0.0, 0.0, u[2 + 3 * NJ], u[3 + 3 * NJ], p[2], p[3]);
+#pragma unroll
+  for (int j = 0; j < NJ; ++j) p[4 + j] = q[j];
+  return had_finish(k, w, xa, xb, p);
+}
+
+// config 4: draws 0-3: s_t, s_t~, s_W+, s_W-; 4-6: gluon; 7-9: y, ln(pT^2 + s_t), phi of t*; 10: y of t~*; 11-18: decays.
+template <bool GRID>
+HG_HD double gen_had_ttxg_dilep(const PsConst& k, uint64_t seed, uint64_t event, uint32_t pid, Mom<double>* p,
+                                uint8_t* bins) {
+  double u[24];
+  draw_uniforms<24>(seed, event, pid, u);
+  double jac = 1.0;
+  if constexpr (GRID) jac = grid_map<24>(k, u, bins);
+  double st, stb, swp, swm;
+  double w = jac * bw_mass(u[0], k.mt, k.mgt, k.tmax_t, st);
+  w *= bw_mass(u[1], k.mt, k.mgt, k.tmax_t, stb);
+  w *= bw_mass(u[2], k.mw, k.mgw, k.tmax_w, swp);
+  w *= bw_mass(u[3], k.mw, k.mgw, k.tmax_w, swm);
+  double y[3], lnpt[3], phi[3], m2[3];
+  y[0] = k.y_jet_max * (2.0 * u[4] - 1.0);
+  lnpt[0] = k.lnpt_lo + (k.lnpt_hi - k.lnpt_lo) * u[5];
+  phi[0] = u[6];
+  w *= (2.0 * k.y_jet_max) * (k.lnpt_hi - k.lnpt_lo);
+  y[1] = k.y_res_max * (2.0 * u[7] - 1.0);
+  const double lt0 = log(st), lt1 = log(st + 0.25 * k.rs * k.rs);   // Eq. 28 from pT = 0 to sqrt(s)/2
+  lnpt[1] = lt0 + (lt1 - lt0) * u[8];
+  phi[1] = u[9];
+  y[2] = k.y_res_max * (2.0 * u[10] - 1.0);
+  w *= (2.0 * k.y_res_max) * (lt1 - lt0) * (2.0 * k.y_res_max);
+  m2[0] = 0.0;
+  m2[1] = st;
+  m2[2] = stb;
+  lnpt[2] = phi[2] = 0.0;
+  Mom<double> q[3];
+  double xa, xb;
+  w *= generalised_ps<3>(y, lnpt, phi, m2, k.rs, q, xa, xb);
+  Mom<double> wp, wm;
+  w *= two_body(q[1], st, k.mb2, swp, u[11], u[12], p[2], wp);
+  w *= two_body(wp, swp, 0.0, 0.0, u[13], u[14], p[3], p[4]);
+  w *= two_body(q[2], stb, k.mb2, swm, u[15], u[16], p[5], wm);
+  w *= two_body(wm, swm, 0.0, 0.0, u[17], u[18], p[6], p[7]);
+  p[8] = q[0];
+  return had_finish(k, w, xa, xb, p);
 }
 
 // ---------------------------------------------------------------- cuts (Eq. 8-11)

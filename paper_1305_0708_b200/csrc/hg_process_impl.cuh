@@ -95,15 +95,18 @@ __global__ void __launch_bounds__(THREADS) me_kernel(const T* __restrict__ p, T*
 // event and me_acc_kernel rebuilds them from its arguments (64 of the 224 + 9 bytes per event of W + 3 jets less
 // to write and read back).  bins (or NULL): [n_draws][n] grid bins of the draws (adaptive-grid steps).
 // GRID: sampling through the adaptive grid k.grid (a separate instantiation: the flat kernel keeps its 72 registers).
-template <class P, class T, class W, bool BEAMS, bool GRID>
+// HAD: the paper's hadronic phase space; the incoming energies then differ from event to event and, with
+// BEAMS = false, are written to beams [2][n] (doubles) for me_acc_kernel.  A point with a null weight (x >= 1) fails.
+template <class P, class T, class W, bool BEAMS, bool GRID, bool HAD>
 __global__ void __launch_bounds__(128) ps_kernel(const PsConst k, uint64_t seed, uint64_t first, int64_t n,
                                                  T* __restrict__ p, W* __restrict__ wps,
-                                                 uint8_t* __restrict__ pass, uint8_t* __restrict__ bins) {
+                                                 uint8_t* __restrict__ pass, uint8_t* __restrict__ bins,
+                                                 double* __restrict__ beams) {
   const int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (e >= n) return;
   Mom<double> q[P::n_ext];
   uint8_t b[GRID ? P::n_draws : 1];
-  const double w = P::template gen<GRID>(k, seed, first + (uint64_t)e, q, GRID && bins ? b : nullptr);
+  const double w = P::template gen<GRID, HAD>(k, seed, first + (uint64_t)e, q, GRID && bins ? b : nullptr);
   constexpr int L0 = BEAMS ? 0 : 2;
 #pragma unroll
   for (int l = L0; l < P::n_ext; ++l) {
@@ -113,7 +116,11 @@ __global__ void __launch_bounds__(128) ps_kernel(const PsConst k, uint64_t seed,
     p[((l - L0) * 4 + 3) * n + e] = T(q[l].z);
   }
   wps[e] = W(w);
-  if (pass) pass[e] = passes_cuts<P>(k, q) ? 1 : 0;
+  if (pass) pass[e] = (passes_cuts<P>(k, q) && (!HAD || w > 0.0)) ? 1 : 0;
+  if constexpr (HAD && !BEAMS) {
+    beams[e] = q[0].e;
+    beams[n + e] = q[1].e;
+  }
   if constexpr (GRID) {
     if (bins) {
 #pragma unroll
@@ -219,14 +226,15 @@ static __global__ void __launch_bounds__(256) compact_kernel(const uint8_t* __re
 // kernels because the phase-space code wants ~70 registers at full occupancy while the staged matrix element
 // runs at 5-6 warps per SM; the round trip through HBM is 32 n_ext + 9 bytes per event against >= 2e4 flops.
 // A block skips me2 only if none of its events passes (every thread must reach the rendezvous inside me2).
-// p holds the final-state legs only (ps_kernel<.., BEAMS = false>); ebeam = sqrt(s_hat)/2.  wout (or NULL): receives
+// p holds the final-state legs only (ps_kernel<.., BEAMS = false>); ebeam = sqrt(s_hat)/2, or beams [2][n] = the
+// energies of the two incoming partons of every event (hadronic phase space).  wout (or NULL): receives
 // the final weight w [pb] of every passing event at its index (adaptive-grid steps: input of hist_kernel).
 template <class P, class T, int THREADS>
 __global__ void __launch_bounds__(THREADS) me_acc_kernel(const T* __restrict__ p, const double* __restrict__ wps,
                                                          const int* __restrict__ idx, const int* __restrict__ cnt,
                                                          int64_t n, int64_t range, const Coup<T> c, double wscale,
-                                                         double ebeam, int add, double* __restrict__ partials,
-                                                         double* __restrict__ wout) {
+                                                         double ebeam, const double* __restrict__ beams, int add,
+                                                         double* __restrict__ partials, double* __restrict__ wout) {
   constexpr int EPB = THREADS / kSplit<P>;
   double sw = 0.0, sw2 = 0.0, np = 0.0;
   const int m = cnt[blockIdx.x];                    // passing events of this block's range, block-uniform
@@ -236,8 +244,9 @@ __global__ void __launch_bounds__(THREADS) me_acc_kernel(const T* __restrict__ p
     const bool ok = j < m;
     const int64_t e = my[ok ? j : m - 1];           // tail lanes recompute the last event (rendezvous inside me2)
     Mom<T> q[P::n_ext];
-    q[0] = mkmom<T>(T(ebeam), T(0), T(0), T(ebeam));
-    q[1] = mkmom<T>(T(ebeam), T(0), T(0), T(-ebeam));
+    const double ea = beams ? beams[e] : ebeam, eb = beams ? beams[n + e] : ebeam;
+    q[0] = mkmom<T>(T(ea), T(0), T(0), T(ea));
+    q[1] = mkmom<T>(T(eb), T(0), T(0), T(-eb));
 #pragma unroll
     for (int l = 2; l < P::n_ext; ++l)
       q[l] = mkmom<T>(p[((l - 2) * 4 + 0) * n + e], p[((l - 2) * 4 + 1) * n + e], p[((l - 2) * 4 + 2) * n + e],
@@ -290,31 +299,36 @@ struct Launch {
     if (prec == HG_F64) return me_t<double>(n, d_p, d_me2, c, s);
     return me_t<float>(n, d_p, d_me2, coup_cast<float>(c), s);
   }
+  // the four (grid, hadronic) variants of the phase-space kernel are separate instantiations
+  template <class T, class W, bool BEAMS>
+  static void ps_launch(unsigned grid, const PsConst& k, uint64_t seed, uint64_t first, int64_t n, T* d_p, W* d_w,
+                        uint8_t* d_pass, uint8_t* d_bins, double* d_beams, cudaStream_t s) {
+    const bool g = k.grid != nullptr, h = k.had != 0;
+    if constexpr (P::has_hadronic) {
+      if (g && h)
+        ps_kernel<P, T, W, BEAMS, true, true><<<grid, 128, 0, s>>>(k, seed, first, n, d_p, d_w, d_pass, d_bins, d_beams);
+      if (!g && h)
+        ps_kernel<P, T, W, BEAMS, false, true><<<grid, 128, 0, s>>>(k, seed, first, n, d_p, d_w, d_pass, d_bins, d_beams);
+    }
+    if (g && !h)
+      ps_kernel<P, T, W, BEAMS, true, false><<<grid, 128, 0, s>>>(k, seed, first, n, d_p, d_w, d_pass, d_bins, d_beams);
+    if (!g && !h)
+      ps_kernel<P, T, W, BEAMS, false, false><<<grid, 128, 0, s>>>(k, seed, first, n, d_p, d_w, d_pass, d_bins, d_beams);
+  }
   static cudaError_t ps(int prec, int64_t n, const PsConst& k, uint64_t seed, uint64_t first, void* d_p,
                         void* d_wps, uint8_t* d_pass, cudaStream_t s) {
     const unsigned grid = (unsigned)((n + 127) / 128);
-    if (prec == HG_F64) {
-      if (k.grid)
-        ps_kernel<P, double, double, true, true><<<grid, 128, 0, s>>>(k, seed, first, n, (double*)d_p,
-                                                                      (double*)d_wps, d_pass, nullptr);
-      else
-        ps_kernel<P, double, double, true, false><<<grid, 128, 0, s>>>(k, seed, first, n, (double*)d_p,
-                                                                       (double*)d_wps, d_pass, nullptr);
-    } else {
-      if (k.grid)
-        ps_kernel<P, float, float, true, true><<<grid, 128, 0, s>>>(k, seed, first, n, (float*)d_p, (float*)d_wps,
-                                                                    d_pass, nullptr);
-      else
-        ps_kernel<P, float, float, true, false><<<grid, 128, 0, s>>>(k, seed, first, n, (float*)d_p, (float*)d_wps,
-                                                                     d_pass, nullptr);
-    }
+    if (prec == HG_F64)
+      ps_launch<double, double, true>(grid, k, seed, first, n, (double*)d_p, (double*)d_wps, d_pass, nullptr, nullptr, s);
+    else
+      ps_launch<float, float, true>(grid, k, seed, first, n, (float*)d_p, (float*)d_wps, d_pass, nullptr, nullptr, s);
     return cudaGetLastError();
   }
   // Layout of the chunk buffer of the split step (context-owned, hg_api.cu): final-state momenta [n_ext - 2][4][chunk]
   // of T | weight double[chunk] | index list int[chunk] | per-block counts int[kMaxPartialBlocks] | pass flags
   // u8[chunk] | adaptive-grid steps only: final weights double[chunk], grid bins u8[n_draws][chunk].
   struct Scratch {   // byte offsets of the sections, each 256-byte aligned
-    size_t p, w, idx, cnt, ok, wout, bins, total;
+    size_t p, w, idx, cnt, ok, beams, wout, bins, total;
   };
   static Scratch scratch_layout(size_t el, int64_t chunk, bool grid) {
     auto up = [](size_t x) { return (x + 255) / 256 * 256; };
@@ -324,7 +338,8 @@ struct Launch {
     L.idx = L.w + up((size_t)chunk * 8);
     L.cnt = L.idx + up((size_t)chunk * 4);
     L.ok = L.cnt + up(sizeof(int) * kMaxPartialBlocks);
-    L.wout = L.ok + up((size_t)chunk);
+    L.beams = L.ok + up((size_t)chunk);
+    L.wout = L.beams + up((size_t)chunk * 16);
     L.bins = L.wout + (grid ? up((size_t)chunk * 8) : 0);
     L.total = L.bins + (grid ? up((size_t)chunk * P::n_draws) : 0);
     return L;
@@ -339,7 +354,7 @@ struct Launch {
     constexpr int TH = int_thr<T>();
     constexpr size_t smem = stage_bytes<P, T, TH>();
     if constexpr (!P::split_step) {
-      if (!k.grid) {   // sampling through a grid always takes the split step (the fused kernel carries no grid code)
+      if (!k.grid && !k.had) {   // grid / hadronic sampling always take the split step (the fused kernel has neither)
         if (ev) cudaEventRecord(ev[0], s);
         integrate_kernel<P, T, TH><<<nblocks, TH, smem, s>>>(k, seed, first, n, c, wscale, d_partials);
         if (ev) cudaEventRecord(ev[2], s);
@@ -355,6 +370,7 @@ struct Launch {
     int* d_idx = (int*)(base + L.idx);
     int* d_cnt = (int*)(base + L.cnt);
     uint8_t* d_ok = (uint8_t*)(base + L.ok);
+    double* d_beams = k.had ? (double*)(base + L.beams) : nullptr;
     double* d_wout = ga ? (double*)(base + L.wout) : nullptr;
     uint8_t* d_bins = ga ? (uint8_t*)(base + L.bins) : nullptr;
     for (int64_t off = 0; off < n; off += chunk) {
@@ -362,16 +378,12 @@ struct Launch {
       const int64_t range = (m + nblocks - 1) / nblocks;
       cudaEvent_t* e3 = ev ? ev + 3 * (off / chunk) : nullptr;
       if (e3) cudaEventRecord(e3[0], s);
-      if (k.grid)
-        ps_kernel<P, T, double, false, true><<<(unsigned)((m + 127) / 128), 128, 0, s>>>(
-            k, seed, first + (uint64_t)off, m, d_p, d_w, d_ok, d_bins);
-      else
-        ps_kernel<P, T, double, false, false><<<(unsigned)((m + 127) / 128), 128, 0, s>>>(
-            k, seed, first + (uint64_t)off, m, d_p, d_w, d_ok, d_bins);
+      ps_launch<T, double, false>((unsigned)((m + 127) / 128), k, seed, first + (uint64_t)off, m, d_p, d_w, d_ok,
+                                  d_bins, d_beams, s);
       compact_kernel<<<nblocks, 256, 0, s>>>(d_ok, m, range, d_idx, d_cnt);
       if (e3) cudaEventRecord(e3[1], s);
       me_acc_kernel<P, T, TH><<<nblocks, TH, smem, s>>>(d_p, d_w, d_idx, d_cnt, m, range, c, wscale, 0.5 * k.rs,
-                                                        off > 0 ? 1 : 0, d_partials, d_wout);
+                                                        d_beams, off > 0 ? 1 : 0, d_partials, d_wout);
       if (e3) cudaEventRecord(e3[2], s);
       if (ga) {
         err = ga->launch(d_bins, d_wout, d_idx, d_cnt, m, range, nblocks, P::n_draws, s);
@@ -403,6 +415,7 @@ struct Launch {
     return prec == HG_F64 ? int_blocks_t<double>(out, split) : int_blocks_t<float>(out, split);
   }
   static bool split_step() { return P::split_step; }
+  static bool has_hadronic() { return P::has_hadronic; }
 };
 
 template <class P>
@@ -410,7 +423,7 @@ constexpr ProcVTable make_vtable(double flops_me, double flops_ps) {
   return ProcVTable{hg_process_info_t{P::n_ext, P::n_final, P::n_hel_total, P::n_hel_nonzero, P::n_diagrams,
                                       P::n_amplitudes, P::n_flows, P::n_draws, P::avg_factor, flops_me, flops_ps},
                     &Launch<P>::me, &Launch<P>::ps, &Launch<P>::integrate, &Launch<P>::int_blocks_per_sm,
-                    &Launch<P>::scratch_bytes, &Launch<P>::split_step};
+                    &Launch<P>::scratch_bytes, &Launch<P>::split_step, &Launch<P>::has_hadronic};
 }
 
 }  // namespace hg

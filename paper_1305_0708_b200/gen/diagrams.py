@@ -166,7 +166,7 @@ class Diagrams:
     def _merge(self, m, nodes):
         groups = {}
         for nd in nodes:
-            key = (nd.field, nd.colour.kind, frozenset(nd.colour.terms))
+            key = (nd.field,) + nd.colour.key()
             groups.setdefault(key, []).append(nd)
         out = []
         for key, grp in groups.items():
@@ -229,7 +229,7 @@ class Diagrams:
         if p.colour == 8:
             return C.leaf('adj', leg.index)
         if abs(p.colour) == 3:
-            return C.leaf('row' if p.is_anti else 'col')
+            return C.leaf('row' if p.is_anti else 'col', leg.index)
         return C.leaf('none')
 
     # ------------------------------------------------------------------ enumeration
@@ -300,7 +300,8 @@ class Diagrams:
                         topo = None
                         for struct in ((1, 2, 3) if v.kind == 'VVVV' else (0,)):
                             try:
-                                col = self._vertex_colour(v, mt[0], [nd.colour for nd in kids], struct)
+                                col = C.closed_flow(self._vertex_colour(v, mt[0], [nd.colour for nd in kids],
+                                                                        struct))
                             except ValueError:
                                 continue
                             if not col.terms:

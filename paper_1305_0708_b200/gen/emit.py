@@ -193,9 +193,15 @@ class CodeGen(Emitter):
     SYNC_EVERY = 1000
     ACC_IN_REGS_MAX = 8   # colour-flow accumulators stay in registers up to this many flows
     SPLIT_SHARED = True   # deal the phases outside the innermost loop to the two warps of a pair
+    # closing by spinor: an FFV vertex that closes on the massless vector leg with one of its spinors independent of
+    # every looped helicity is evaluated as a dot product with that spinor dressed once per event (hg_helas.cuh
+    # dress_row / dress_col / sdot) instead of current + projection
+    DRESS = True
 
-    def __init__(self, diag, stage=False, kfromp=False):
+    def __init__(self, diag, stage=False, kfromp=False, dress=None):
         super().__init__(diag)
+        if dress is not None:
+            self.DRESS = dress
         self.stage = stage
         self.kfromp = stage and kfromp   # inside loops rebuild internal momenta from staged external momenta
 
@@ -307,7 +313,7 @@ class CodeGen(Emitter):
         return out
 
     # rough cost (flops) of an emitted call, used only to balance the two halves of a shared phase
-    _CALL_COST = (('fvixxx', 63), ('fvoxxx', 63), ('fsixxx', 40), ('fsoxxx', 40), ('jioxx', 45), ('jvvxxx', 110),
+    _CALL_COST = (('dress_', 45), ('fvixxx', 63), ('fvoxxx', 63), ('fsixxx', 40), ('fsoxxx', 40), ('jioxx', 45), ('jvvxxx', 110),
                   ('jgggxx', 70), ('vxxxxx', 40), ('ixxxx0', 25), ('oxxxx0', 25), ('crcp', 25), ('hrcp', 15),
                   ('unit0', 18), ('two_dot0', 8))
 
@@ -671,9 +677,13 @@ class CodeGen(Emitter):
             self._begin(k)
             lines = []
             if cbc:
-                lines.append('const Vc<T> b = %s;' % self._root_current_expr(rt, vi, hel))
-                lines.append('cx<T> rb, ib;')
-                lines.append('close_proj(%s, b, rb, ib);' % self._ref('e%d' % last))
+                dressed = self._dressed_closing(rt, vi, hel, k)
+                if dressed:
+                    lines += dressed
+                else:
+                    lines.append('const Vc<T> b = %s;' % self._root_current_expr(rt, vi, hel))
+                    lines.append('cx<T> rb, ib;')
+                    lines.append('close_proj(%s, b, rb, ib);' % self._ref('e%d' % last))
                 for w, cf in sorted(rt.colour.terms.items()):
                     f = fidx[w]
                     if acc_smem:
@@ -728,6 +738,49 @@ class CodeGen(Emitter):
         else:
             accdecl = 'cx<T> ' + ', '.join('j%d = czero<T>()' % f for f in range(nf)) + ';'
         return dict(hel=hel, levels=levels, tail=tail, k=k, accdecl=accdecl)
+
+    def _dressed_closing(self, rt, vi, hel, k):
+        """Lines that compute rb, ib of an FFV root as spinor dot products, or None if neither spinor is helicity-loop
+        independent (or the option is off).  The dressed spinors are depth-0 values, defined once and shared."""
+        if not self.DRESS or rt.vertex.kind != 'FFV' or k == 0:
+            return None
+        v = rt.vertex
+        by_slot = dict(zip(rt.slots, rt.children))
+        row, col = by_slot[0], by_slot[1]
+        drow, dcol = self._depth(row.mask), self._depth(col.mask)
+        if min(drow, dcol) != 0 or max(drow, dcol) == 0:
+            return None
+        g = self._gmask(v)
+        mrow, mcol = self._node_mask(row, hel, self.memo), self._node_mask(col, hel, self.memo)
+        left = bool((mcol & A) and (mrow & B) and (g & GL))
+        right = bool((mcol & B) and (mrow & A) and (g & GR))
+        if not (left or right):
+            return None
+        last = self.dg.last
+        gl, gr = self._cpl(v.coup[0]), self._cpl(v.coup[1])
+        if drow == 0:     # dress the row spinor; its L part lands in slots A (meets the column's slots A)
+            base, fn, m_in = self._name(row, vi, hel), 'dress_row', mrow
+            dmask = (A if left else 0) | (B if right else 0)
+            other = col
+        else:             # dress the column spinor; its L part lands in slots B (meets the row's slots B)
+            base, fn, m_in = self._name(col, vi, hel), 'dress_col', mcol
+            dmask = (B if left else 0) | (A if right else 0)
+            other = row
+        names = []
+        for part, tag in ((0, 'zr'), (1, 'zi')):
+            name = '%s_%s_%s' % (tag, base, (v.coup[0] or '0') + (v.coup[1] or '0'))
+            if name not in self.shared:
+                self._reg(name, 'Sp<T>', 0, mask=dmask)
+                self._begin(0)
+                expr = '%s<%d, %d, %d>(%s, %s, %s, %s)' % (fn, m_in, g, part, self._ref(base), self._ref('e%d' % last),
+                                                          gl, gr)
+                self.shared[name] = True
+                self.shared_items.append(('def', name, expr, self.cur_loads))
+            names.append(name)
+        self._begin(k)
+        o = self._ref(self._name(other, vi, hel))
+        zr, zi = self._ref(names[0]), self._ref(names[1])
+        return ['const cx<T> rb = sdot<%d>(%s, %s), ib = sdot<%d>(%s, %s);' % (dmask, zr, o, dmask, zi, o)]
 
     def _render_variant(self, var):
         dyn = self.dynamic

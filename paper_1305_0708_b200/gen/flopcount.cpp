@@ -16,6 +16,8 @@
 #include "../csrc/generated/hg_proc_7.cuh"
 #include "../csrc/generated/hg_proc_8.cuh"
 #include "../csrc/generated/hg_proc_9.cuh"
+#include "../csrc/generated/hg_proc_10.cuh"
+#include "../csrc/generated/hg_proc_11.cuh"
 
 using namespace hg;
 
@@ -62,5 +64,7 @@ int main() {
   run<P7>(1000.0);
   run<P8>(1000.0);
   run<P9>(3000.0);
+  run<P10>(1000.0);
+  run<P11>(1000.0);
   return 0;
 }

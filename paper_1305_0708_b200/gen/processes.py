@@ -22,10 +22,17 @@ SPECS = [
     ProcessSpec('gg_ttxh', 8, ['g', 'g'], ['t', 't~', 'h']),
     # next size up: W + 4 jets, 428 diagrams / 516 amplitudes, 24 colour flows
     ProcessSpec('udx_epvegggg', 9, ['u', 'd~'], ['e+', 've', 'g', 'g', 'g', 'g']),
+    # weak-boson fusion, two quark lines (Eq. 21a, 22a): W W and Z Z
+    # fusion interfere (different colour flows, relative Fermi sign); VVS, and VVS + VVSS + SSS
+    ProcessSpec('ud_hud', 10, ['u', 'd'], ['h', 'u', 'd']),
+    ProcessSpec('ud_hhud', 11, ['u', 'd'], ['h', 'h', 'u', 'd']),
 ]
 
+# resonance of the W/Z + jets family in the paper's hadronic phase space: suffix of PsConst::m?, mg?, tmax_?
+HADRONIC = {1: 'w', 2: 'z', 3: 'w', 5: 'w', 9: 'w'}
+
 # uniform random numbers per event used by the phase-space generator
-N_DRAWS = {1: 8, 2: 12, 3: 16, 4: 24, 5: 20, 6: 12, 7: 16, 8: 12, 9: 24}
+N_DRAWS = {1: 8, 2: 12, 3: 16, 4: 24, 5: 20, 6: 12, 7: 16, 8: 12, 9: 24, 10: 12, 11: 16}
 
 # rough per-call cost (flops) used only to choose the closing leg; the reported flop counts are measured by
 # running the generated code on a counting type (gen/flopcount.py)
@@ -74,6 +81,9 @@ MERGE = True
 # of those, processes that rebuild internal momenta from staged external momenta inside the loops (fewer slots,
 # more shared-memory loads)
 KFROMP = set()
+# processes whose FFV closings do NOT go through dressed spinors (gen/emit.py DRESS): config 4 would need 174 staged
+# words instead of 142 and fall from 12 to 8 warps per SM
+NO_DRESS = {4}
 
 
 def build(spec, last=None):
@@ -82,7 +92,8 @@ def build(spec, last=None):
     if last is None:
         last = spec.last
     def make(leg):
-        cg_ = CodeGen(Diagrams(spec, merge=MERGE).build(leg), stage, spec.pid in KFROMP)
+        cg_ = CodeGen(Diagrams(spec, merge=MERGE).build(leg), stage, spec.pid in KFROMP,
+                      dress=spec.pid not in NO_DRESS)
         cg_.count_dg = Diagrams(spec).build(leg)   # Feynman-diagram counts: the unmerged enumeration
         return cg_
 
@@ -174,6 +185,15 @@ def render_descriptor(cg):
             len(spec.final), spec.pid, ', '.join('k.%s' % m if m else '0.0' for m in fmass))
     else:
         gen_call = 'gen_massless<%d, GRID>(k, seed, event, %d, p, bins)' % (len(spec.final), spec.pid)
+    # the paper's hadronic phase space (hg_set_hadronic, reading A23): W/Z + jets family and config 4
+    res = HADRONIC.get(spec.pid)
+    if spec.decays:
+        had_call = 'gen_had_ttxg_dilep<GRID>(k, seed, event, %d, p, bins)' % spec.pid
+    elif res:
+        had_call = 'gen_had_vjets<%d, %d, GRID>(k, seed, event, %d, k.m%s, k.mg%s, k.tmax_%s, p, bins)' % (
+            len(jets), N_DRAWS[spec.pid], spec.pid, res, res, res)
+    else:
+        had_call = None
     return """// GENERATED by paper_1305_0708_b200/gen (python -m paper_1305_0708_b200.gen) -- do not edit.
 // process %(pid)d: %(proc)s
 #pragma once
@@ -200,9 +220,15 @@ struct P%(pid)d {
     return t[i];
   }
   // GRID: sample through the adaptive grid k.grid; bins (or NULL) then receives the grid bin of every draw
-  template <bool GRID = false>
+  // HAD: the paper's hadronic phase space (k.rs = hadronic sqrt(s)) instead of RAMBO at fixed s_hat
+  static constexpr bool has_hadronic = %(has_had)s;
+  template <bool GRID = false, bool HAD = false>
   HG_HD static double gen(const PsConst& k, uint64_t seed, uint64_t event, Mom<double>* p, uint8_t* bins = nullptr) {
-    return %(gen_call)s;
+    if constexpr (HAD) {
+      %(had_call)s
+    } else {
+      return %(gen_call)s;
+    }
   }
   template <class T, class St>
   HG_HD static T me2(const Mom<T>* p, const Coup<T>& c, const St& st) {
@@ -216,7 +242,8 @@ struct P%(pid)d {
            n_flows=row['n_flows'], n_draws=row['n_draws'], n_stage=cg.n_stage,
            split_step='true' if (cg.n_stage > 0 or spec.pid in SPLIT_STEP) else 'false', avg=repr(row['avg_factor']),
            me_threads=ME_THREADS.get(spec.pid, 128), n_jets=len(jets), n_leps=len(leps), jets=arr(jets),
-           leps=arr(leps), gen_call=gen_call)
+           leps=arr(leps), gen_call=gen_call, has_had='true' if had_call else 'false',
+           had_call=('return %s;' % had_call) if had_call else 'return 0.0;  // not implemented: rejected by the C ABI')
 
 
 def render_unit(spec, flops_me, flops_ps):
@@ -232,7 +259,7 @@ extern const ProcVTable hg_proc_%(pid)d = make_vtable<P%(pid)d>(%(fme)r, %(fps)r
 
 
 # threads per block of the matrix-element kernel (tuned with ncu)
-ME_THREADS = {1: 256, 2: 128, 3: 128, 4: 128, 5: 128, 6: 128, 7: 128, 8: 128, 9: 128}
+ME_THREADS = {1: 256, 2: 128, 3: 128, 4: 128, 5: 128, 6: 128, 7: 128, 8: 128, 9: 128, 10: 128, 11: 128}
 
 
 def count_flops(outdir):

@@ -14,7 +14,8 @@ import torch
 
 from . import api
 
-SQRT_S = {1: 80.0, 2: 500.0, 3: 1000.0, 4: 1500.0, 5: 2000.0, 6: 500.0, 7: 1000.0, 8: 1000.0, 9: 3000.0}
+SQRT_S = {1: 80.0, 2: 500.0, 3: 1000.0, 4: 1500.0, 5: 2000.0, 6: 500.0, 7: 1000.0, 8: 1000.0, 9: 3000.0, 10: 1000.0,
+          11: 1000.0}
 
 
 def run(processes, n, big=False, seed=13050708):

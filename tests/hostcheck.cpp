@@ -17,6 +17,8 @@
 #include "../paper_1305_0708_b200/csrc/generated/hg_proc_7.cuh"
 #include "../paper_1305_0708_b200/csrc/generated/hg_proc_8.cuh"
 #include "../paper_1305_0708_b200/csrc/generated/hg_proc_9.cuh"
+#include "../paper_1305_0708_b200/csrc/generated/hg_proc_10.cuh"
+#include "../paper_1305_0708_b200/csrc/generated/hg_proc_11.cuh"
 
 using namespace hg;
 
@@ -48,6 +50,8 @@ int main() {
       case 7: ok = eval<P7>(c); break;
       case 8: ok = eval<P8>(c); break;
       case 9: ok = eval<P9>(c); break;
+      case 10: ok = eval<P10>(c); break;
+      case 11: ok = eval<P11>(c); break;
     }
     if (!ok) return 1;
   }

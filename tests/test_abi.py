@@ -32,8 +32,11 @@ def test_process_info_matches_survey_table(api):
     expect = {1: (4, 16, 1, 1, 1, 1), 2: (5, 32, 8, 4, 4, 1), 3: (6, 64, 4, 8, 8, 2), 4: (9, 512, 8, 16, 18, 6),
               5: (7, 128, 8, 50, 54, 6),
               # NEXT-1 / NEXT-4 processes; a scalar leg has one state
-              6: (5, 16, 1, 1, 1, 1), 7: (6, 16, 4, 4, 4, 1), 8: (5, 16, 16, 8, 8, 2), 9: (8, 256, 16, 428, 516, 24)}
-    avg = {1: 1 / 36, 2: 1 / 36, 3: 1 / 72, 4: 1 / 256, 5: 1 / 216, 6: 1 / 36, 7: 1 / 72, 8: 1 / 256, 9: 1 / 864}
+              6: (5, 16, 1, 1, 1, 1), 7: (6, 16, 4, 4, 4, 1), 8: (5, 16, 16, 8, 8, 2), 9: (8, 256, 16, 428, 516, 24),
+              # weak-boson fusion, two quark lines: W W and Z Z fusion = two colour flows
+              10: (5, 16, 4, 2, 2, 2), 11: (6, 16, 4, 8, 8, 2)}
+    avg = {1: 1 / 36, 2: 1 / 36, 3: 1 / 72, 4: 1 / 256, 5: 1 / 216, 6: 1 / 36, 7: 1 / 72, 8: 1 / 256, 9: 1 / 864,
+           10: 1 / 36, 11: 1 / 72}
     for pid, e in expect.items():
         i = api.hg_process_info(pid)
         assert (i['n_ext'], i['n_hel_total'], i['n_hel_nonzero'], i['n_diagrams'], i['n_amplitudes'],

@@ -16,7 +16,7 @@ from oracle import sm as osm
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 SRC = os.path.join(ROOT, 'tests', 'hostcheck.cpp')
-N = {1: 64, 2: 48, 3: 24, 4: 4, 5: 6, 6: 64, 7: 48, 8: 48, 9: 3}
+N = {1: 64, 2: 48, 3: 24, 4: 4, 5: 6, 6: 64, 7: 48, 8: 48, 9: 3, 10: 48, 11: 48}
 
 
 @pytest.fixture(scope='module')
@@ -26,7 +26,7 @@ def exe(tmp_path_factory):
     return out
 
 
-@pytest.mark.parametrize('cfg', [1, 2, 3, 4, 5, 6, 7, 8, 9])
+@pytest.mark.parametrize('cfg', [1, 2, 3, 4, 5, 6, 7, 8, 9, 10, 11])
 def test_generated_code_matches_oracle(exe, cfg):
     par = osm.default_params()
     p, _ = ops.generate(cfg, 7, 0, N[cfg], opr.SQRT_S[cfg], par)

@@ -24,10 +24,10 @@ SEED = 13050708
 # Events per config for the element-by-element comparison (SURVEY.md 8c parity protocol: the first 65,536 events of
 # the stream for the small processes, >= 4,096 for configs 4 and 5, >= 512 for W + 4 jets; all sizes are ragged:
 # whole blocks plus a tail).  The oracle runs over the host cores (tests/oracle_pool.py).
-N_PARITY = {1: 65536, 2: 65539, 3: 65539, 4: 4099, 5: 4099, 6: 65539, 7: 65539, 8: 16387, 9: 515}
+N_PARITY = {1: 65536, 2: 65539, 3: 65539, 4: 4099, 5: 4099, 6: 65539, 7: 65539, 8: 16387, 9: 515, 10: 65539, 11: 16387}
 N_EDGE = 1024                    # edge stress: the passing events with the smallest min(s_ij) of 2^20 points
-ALL = [1, 2, 3, 4, 5, 6, 7, 8, 9]  # 6-8: Higgs-sector processes (NEXT-1); 9: W + 4 jets (NEXT-4)
-MASSIVE_PS = (4, 6, 7, 8)        # phase space with a Newton solve (massive RAMBO)
+ALL = [1, 2, 3, 4, 5, 6, 7, 8, 9, 10, 11]  # 6-8, 10, 11: Higgs-sector processes (NEXT-1); 9: W + 4 jets (NEXT-4)
+MASSIVE_PS = (4, 6, 7, 8, 10, 11)        # phase space with a Newton solve (massive RAMBO)
 STAGED = (4, 5, 9)               # processes whose matrix element runs staged and pair-split
 
 
@@ -549,34 +549,111 @@ def test_grid_sampling_matches_oracle(ctx, api, cfg):
     assert np.abs(q.cpu().numpy().transpose(2, 0, 1) - p0).max() <= 1e-9 * rs
 
 
-def test_grid_adaptation_reduces_the_variance(ctx, api):
-    """Grid optimisation (5 iterations of 2^20 points: step with histogram -> hg_grid_refine) then an integration
-    step, W + 3 jets: the estimates of all iterations agree within errors, and the adapted grid has a smaller
-    Monte-Carlo error per point than flat sampling.  The same loop in the oracle (small) follows the same grid."""
+def _had_dict(h):
+    return dict(y_res_max=h.y_res_max, pdf_norm=tuple(h.pdf_norm), pdf_a=tuple(h.pdf_a), pdf_b=tuple(h.pdf_b))
+
+
+@pytest.mark.parametrize('cfg', [1, 2, 3, 4, 5, 9])
+def test_hadronic_phase_space_matches_oracle(ctx, api, cfg):
+    """The paper's own phase space (Eq. 24-28, App. A; hg_set_hadronic) at sqrt(s) = 14 TeV with the toy parton
+    densities: momenta, weights, pass flags (x < 1 and the cuts) against oracle/phase_space_had.py, |Mbar|^2 at those
+    lab-frame momenta against the oracle, and the sums of the step."""
+    from oracle import phase_space_had as ohad
+    n, rs = (1283 if cfg != 9 else 131), 14000.0
+    h = api.hg_default_hadronic(cfg)
+    p_ref, w_ref, valid = ohad.generate(cfg, SEED, 5, n, rs, PAR, _had_dict(h))
+    ok_ref = ops.passes(cfg, p_ref) & valid
+    try:
+        ctx.hg_set_hadronic(h)
+        p, w, ok = ctx.hg_gen_phase_space(cfg, api.HG_F64, SEED, 5, n, rs)
+        me = ctx.hg_matrix_element(cfg, api.HG_F64, p).cpu().numpy()
+        acc = ctx.hg_integrate_step(cfg, api.HG_F64, SEED, 5, n, rs)
+        acc32 = ctx.hg_integrate_step(cfg, api.HG_F32, SEED, 5, n, rs)
+        a = ctx.hg_integrate_step(cfg, api.HG_F64, SEED, 5, n // 2, rs)
+        b = ctx.hg_integrate_step(cfg, api.HG_F64, SEED, 5 + n // 2, n - n // 2, rs)
+        with pytest.raises(api.HgError):
+            ctx.hg_integrate_step(6, api.HG_F64, SEED, 0, 10, rs)      # not implemented for the Higgs processes
+    finally:
+        ctx.hg_set_hadronic(None)
+    p = p.cpu().numpy().transpose(2, 0, 1)
+    w = w.cpu().numpy()
+    ok = ok.cpu().numpy().astype(bool)
+    scale = np.abs(p_ref).reshape(n, -1).max(1)
+    assert np.all(np.abs(p - p_ref).reshape(n, -1).max(1) <= 1e-12 * scale)
+    # (1 - x)^b of the toy densities amplifies the rounding of x by b / (1 - x): relative bound away from x = 1,
+    # absolute bound (on the scale of the largest weight) near it
+    assert np.allclose(w, w_ref, rtol=1e-11, atol=1e-13 * w_ref.max())
+    assert (np.count_nonzero(valid) < n or cfg == 1) and np.all(w[~valid] == 0)
+    assert np.array_equal(ok, ok_ref)
+    sel = np.nonzero(ok_ref)[0]
+    assert len(sel) > n // 10
+    # In the lab frame the incoming partons carry very different energies (x_a ~ 0.1, x_b ~ 0.001): the fp64 oracle
+    # forms invariants as E^2 - |p|^2 of boosted momenta and is good to ~1e-10 only, so the arbiter (same formulas in
+    # extended precision, reading A21) is the reference for every event; against it the flat 1e-11 holds.
+    ref = oracle_pool.me2(cfg, p_ref[sel], PAR, extended=True)
+    rel = np.abs(me[sel] - ref) / ref
+    # flat 1e-11, except where the input itself fixes |M|^2 less well: config 1 vanishes at cos(theta) = -1 (the
+    # invariant p_u . p_e+ -> 0) and has no cut that keeps events away from that zero; one ulp of a momentum moves a
+    # small invariant by eps * s_max / s_min (assert_fp64_parity)
+    ps_ = p_ref[sel]
+    big = np.zeros(len(sel))
+    for a_ in range(ps_.shape[1]):
+        for b_ in range(a_ + 1, ps_.shape[1]):
+            d_ = ps_[:, a_, 0] * ps_[:, b_, 0] - (ps_[:, a_, 1:] * ps_[:, b_, 1:]).sum(1)
+            big = np.maximum(big, 2 * np.abs(d_))
+    tol = np.maximum(1e-11, 4 * np.finfo(float).eps * big / min_invariant(ps_)) if cfg == 1 else 1e-11
+    assert np.all(rel <= tol), (cfg, float(rel.max()))
+    ref64 = oracle_pool.me2(cfg, p_ref[sel], PAR)
+    assert np.abs(ref64 - ref).max() <= 1e-8 * ref.max() and np.median(np.abs(ref64 - ref) / ref) < 1e-11
+    wt = np.zeros(n)
+    wt[sel] = ref * w_ref[sel] / (2 * rs * rs) * osm.HBARC2_PB
+    want = oint.accumulate(wt, ok_ref)
+    assert acc[3] == want[3] and acc[2] == n
+    assert abs(acc[0] - want[0]) <= 1e-10 * want[0] and abs(acc[1] - want[1]) <= 2e-10 * want[1]
+    assert acc32[3] == acc[3] and abs(acc32[0] - acc[0]) <= 1e-4 * acc[0]
+    assert a[3] + b[3] == acc[3] and abs(a[0] + b[0] - acc[0]) <= 1e-12 * acc[0]
+    # back to RAMBO at fixed s_hat
+    q, _, _ = ctx.hg_gen_phase_space(cfg, api.HG_F64, SEED, 3, 8, opr.SQRT_S[cfg])
+    p0, _ = ops.generate(cfg, SEED, 3, 8, opr.SQRT_S[cfg], PAR)
+    assert np.abs(q.cpu().numpy().transpose(2, 0, 1) - p0).max() <= 1e-9 * opr.SQRT_S[cfg]
+
+
+def _adapt(ctx, api, cfg, rs, n, iters, alpha, nb):
+    """Grid optimisation: `iters` steps with histogram + hg_grid_refine, then one integration step on the final grid."""
     from oracle import vegas
-    cfg, rs, nb, n = 5, 2000.0, 50, 1 << 20
     nd = ops.N_DRAWS[cfg]
     grid = torch.from_numpy(vegas.uniform_grid(nd, nb)).contiguous()
-    flat = ctx.hg_integrate_step(cfg, api.HG_F64, SEED, 0, n, rs)
-    s0, e0 = oint.sigma(flat)
-    ests = [(s0, e0)]
+    ests = []
     try:
-        for it in range(5):
-            d_grid = grid.cuda()
+        for it in range(iters):
             d_hist = torch.zeros((nd, nb), dtype=torch.float64, device='cuda')
-            ctx.hg_set_grid(d_grid, d_hist)
-            acc = ctx.hg_integrate_step(cfg, api.HG_F64, SEED, (it + 1) * n, n, rs)
-            ests.append(oint.sigma(acc))
-            api.hg_grid_refine(d_hist.cpu(), 1.5, grid)
+            ctx.hg_set_grid(grid.cuda(), d_hist)
+            ests.append(oint.sigma(ctx.hg_integrate_step(cfg, api.HG_F64, SEED, (it + 1) * n, n, rs)))
+            api.hg_grid_refine(d_hist.cpu(), alpha, grid)
         ctx.hg_set_grid(grid.cuda(), None)
-        final = ctx.hg_integrate_step(cfg, api.HG_F64, SEED, 7 * n, n, rs)
+        final = ctx.hg_integrate_step(cfg, api.HG_F64, SEED, (iters + 2) * n, n, rs)
     finally:
         ctx.hg_set_grid(None)
-    s1, e1 = oint.sigma(final)
-    assert abs(s1 - s0) <= 4 * math.hypot(e0, e1), (s0, e0, s1, e1)
-    for s_, e_ in ests[2:]:
-        assert abs(s_ - s1) <= 5 * math.hypot(e_, e1)
-    assert e1 < 0.7 * e0, (e0, e1)
-    # grid edges stay a valid partition
     g = grid.numpy()
     assert np.all(np.diff(g, axis=1) > 0) and np.all(g[:, 0] == 0) and np.all(g[:, -1] == 1)
+    return ests, final
+
+
+def test_grid_adaptation_reduces_the_variance(ctx, api):
+    """BASES-style integration: grid optimisation then an integration step, W + 3 jets in the
+    paper's own variables (y, ln pT^2, phi: aligned with the soft / collinear structure of the integrand), 5 iterations
+    of 2^20 points: the Monte-Carlo error per point drops by more than 3 and the estimates agree.  (On flat RAMBO
+    variables, which are not aligned with the soft / collinear structure, the same loop does not help -- measured, see
+    DESIGN.md section 9: that is the paper's argument for its parameterisation.)"""
+    cfg, rs, n = 5, 14000.0, 1 << 20
+    try:
+        ctx.hg_set_hadronic(api.hg_default_hadronic(cfg))
+        flat = ctx.hg_integrate_step(cfg, api.HG_F64, SEED, 0, n, rs)
+        ests, final = _adapt(ctx, api, cfg, rs, n, 5, 1.0, 50)
+    finally:
+        ctx.hg_set_hadronic(None)
+    s0, e0 = oint.sigma(flat)
+    s1, e1 = oint.sigma(final)
+    assert abs(s1 - s0) <= 4 * math.hypot(e0, e1), (s0, e0, s1, e1)
+    assert e1 < e0 / 3, (e0, e1, ests)
+    assert final[3] / final[2] > 0.9 * flat[3] / flat[2]        # the pass fraction does not collapse

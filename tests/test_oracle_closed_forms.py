@@ -219,3 +219,59 @@ def test_w_plus_one_gluon_soft_limit_onto_cfg1():
             (48 * ((s - PAR['mw'] ** 2) ** 2 + (PAR['mw'] * PAR['gw']) ** 2))
         devs.append(np.max(np.abs(m3 / (eik * cf) - 1)))
     assert devs[0] < 5e-3 and devs[1] < 5e-5, devs
+
+
+def test_four_quark_closed_forms_fix_the_fermi_sign():
+    """Two quark lines: textbook massless QCD 2 -> 2 results.  q q' -> q q' has one diagram; q q -> q q and
+    q q~ -> q q~ have two whose fermion lines pair the external legs differently: their interference carries the
+    relative Fermi sign (oracle.feynman.fermion_sign) and the colour-suppressed factor.  With the wrong sign the
+    interference term flips: the ratios below are off by 20-60 %."""
+    from oracle import feynman as fy
+    gs4 = sm.couplings(PAR)['gs'] ** 4
+    p = inputs.two_to_two(500.0, 0.0, 0.0, 16, seed=3, cmax=0.8)
+    s, t, u = inputs.mandelstam(p)
+    cases = [
+        (P.Process('ud_ud', ['u', 'd'], ['u', 'd'], ['uug', 'ddg']), (4 / 9) * (s * s + u * u) / (t * t)),
+        (P.Process('uu_uu', ['u', 'u'], ['u', 'u'], ['uug']),
+         ((4 / 9) * ((s * s + u * u) / (t * t) + (s * s + t * t) / (u * u)) - (8 / 27) * s * s / (t * u)) / 2),
+        (P.Process('uux_uux', ['u', 'u~'], ['u', 'u~'], ['uug']),
+         (4 / 9) * ((s * s + u * u) / (t * t) + (t * t + u * u) / (s * s)) - (8 / 27) * u * u / (s * t)),
+        (P.Process('uux_ddx', ['u', 'u~'], ['d', 'd~'], ['uug', 'ddg']), (4 / 9) * (t * t + u * u) / (s * s)),
+    ]
+    for proc, want in cases:
+        got = P.me2(proc, p, PAR)
+        assert np.allclose(got, gs4 * want, rtol=1e-12), proc.name
+        assert np.allclose(P.me2_explicit_colour(proc, p[:3], PAR), got[:3], rtol=1e-12)
+    roots = cases[2][0].diagrams(PAR)[0]
+    assert sorted(fy.fermion_sign(r) for r in roots) == [-1, 1]
+    assert [len(fy.fermion_lines(r)) for r in roots] == [2, 2]
+
+
+def test_ww_fusion_closed_form():
+    """u b -> h d t is pure t-channel W W fusion (one diagram: Z Z fusion would leave u b in the final state).  With
+    the W W H coupling g_W m_W and left-handed currents,
+        sum |M|^2 = (g_W^2/2)^2 (g_W m_W)^2 16 (p_u.p_b)(p_d.p_t) / (|D_1|^2 |D_2|^2),
+    colour 9, average 1/36; D_i = q_i^2 - m_W^2 + i m_W Gamma_W on the space-like lines.  The top is taken massless
+    here (t and b merely stand for a second quark doublet): with m_t != 0 the q_mu q_nu / m_W^2 term of the
+    unitary-gauge propagator contributes through the non-conserved t b current."""
+    par = dict(PAR, mt=0.0, gt=0.0)
+    proc = P.Process('ub_hdt', ['u', 'b'], ['h', 'd', 't'], ['udw', 'tbw', 'wwh'])
+    assert len(proc.diagrams(par)[0]) == 1
+    from oracle import phase_space as ops
+    from oracle import philox
+    n, rs = 32, 1000.0
+    u = philox.uniforms(5, 0, n, 12, 3)
+    masses = np.stack([np.full(n, PAR['mh']), np.zeros(n), np.zeros(n)], 1)
+    k, _ = ops.rambo_massive(u, masses, rs)
+    p = np.zeros((n, 5, 4))
+    p[:, 0] = [rs / 2, 0, 0, rs / 2]
+    p[:, 1] = [rs / 2, 0, 0, -rs / 2]
+    p[:, 2:] = k
+    gw, mw, gam = sm.couplings(PAR)['gw'], PAR['mw'], PAR['gw']
+    q1 = p[:, 0] - p[:, 3]
+    q2 = p[:, 1] - p[:, 4]
+    d1 = (inputs.mdot(q1, q1) - mw * mw) ** 2 + (mw * gam) ** 2
+    d2 = (inputs.mdot(q2, q2) - mw * mw) ** 2 + (mw * gam) ** 2
+    want = (gw ** 2 / 2) ** 2 * (gw * mw) ** 2 * 16 * inputs.mdot(p[:, 0], p[:, 1]) * inputs.mdot(p[:, 3], p[:, 4]) \
+        / (d1 * d2) * 9 / 36
+    assert np.allclose(P.me2(proc, p, par), want, rtol=1e-11)

@@ -165,7 +165,7 @@ def test_ward_identity_gg_ttxh():
         assert _ward_residual(proc, p, par, leg) < 1e-22
 
 
-@pytest.mark.parametrize("cfg", [6, 7, 8])
+@pytest.mark.parametrize("cfg", [6, 7, 8, 10, 11])
 def test_lorentz_invariance_higgs_processes(cfg):
     par = dict(PAR, gt=0.0) if cfg == 8 else PAR
     proc = P.config(cfg)
@@ -199,3 +199,25 @@ def test_w4j_counts_and_ward_identity():
     # a^dagger C a with 516 terms that cancel among themselves: rounding leaves ~1e-15 of the physical value; a wrong
     # sign or colour factor anywhere leaves O(1e-3 .. 1)
     assert np.max(P.me2(proc, p, PAR, wf_hook=hook) / P.me2(proc, p, PAR)) < 1e-12
+
+
+def test_weak_boson_fusion_structure():
+    """u d -> h u d and u d -> h h u d (processes 10, 11): diagram counts, the two pairings of the quark legs with
+    opposite Fermi sign, the colour matrix [[9, 3], [3, 9]] of the two pairings from the brute-force index sum, the
+    explicit colour sum, and Bose symmetry of the two Higgs bosons."""
+    from oracle import feynman as fy
+    for cfg, ndiag in ((10, 2), (11, 8)):
+        proc = P.config(cfg)
+        roots, cm, _ = proc.diagrams(PAR)
+        assert len(roots) == ndiag
+        pairings = {tuple(fy.fermion_lines(r)): fy.fermion_sign(r) for r in roots}
+        assert len(pairings) == 2 and sorted(pairings.values()) == [-1, 1]
+        vals = sorted(set(np.round(cm.real.reshape(-1), 10)))
+        assert vals == [3.0, 9.0] and np.abs(cm.imag).max() == 0
+        p = ps.generate(cfg, 78, 0, 4, P.SQRT_S[cfg], PAR)[0]
+        m = P.me2(proc, p, PAR)
+        assert np.allclose(P.me2_explicit_colour(proc, p, PAR), m, rtol=1e-12)
+        if cfg == 11:
+            q = p.copy()
+            q[:, [2, 3]] = p[:, [3, 2]]
+            assert np.max(np.abs(P.me2(proc, q, PAR) / m - 1)) < 1e-12
