@@ -160,6 +160,34 @@ def time_oracle(cfg, steps, warmup, n=None, all_cores=True):
         wall / steps
 
 
+def time_generated_host(cfg, n_events):
+    """The generated matrix elements + phase space compiled for the host (gen/hoststep.cpp, g++ -O3 -fopenmp) on all
+    cores: a compiled CPU implementation of the same algorithm, the counterpart of the paper's Fortran HELAS baseline.
+    An extra, labelled figure; `cpu_baseline` stays the oracle."""
+    import tempfile
+    src = os.path.join(ROOT, 'paper_1305_0708_b200', 'gen', 'hoststep.cpp')
+    try:
+        with tempfile.TemporaryDirectory() as tmp:
+            exe = os.path.join(tmp, 'hoststep')
+            subprocess.check_call(['g++', '-O3', '-march=native', '-fopenmp', '-std=c++17', src, '-o', exe, '-lm'],
+                                  stderr=subprocess.DEVNULL)
+            env = {k_: v_ for k_, v_ in os.environ.items() if k_ != 'OMP_NUM_THREADS'}      # all cores
+            subprocess.check_output([exe, str(cfg), repr(SQRT_S[cfg]), str(SEED), '0', str(n_events // 8)], env=env)
+            out = subprocess.check_output([exe, str(cfg), repr(SQRT_S[cfg]), str(SEED), '0', str(n_events)],
+                                          text=True, env=env).split()
+            env1 = dict(os.environ, OMP_NUM_THREADS='1')
+            out1 = subprocess.check_output([exe, str(cfg), repr(SQRT_S[cfg]), str(SEED), '0', str(n_events // 8)],
+                                           text=True, env=env1).split()
+    except (OSError, subprocess.CalledProcessError) as e:
+        return {'unavailable': 'g++ build or run of gen/hoststep.cpp failed: %r' % (e,)}
+    sec, threads = float(out[3]), int(out[4])
+    return {'value': n_events / sec, 'unit': UNIT, 'cores': threads, 'kind': 'generated code on the host',
+            'value_1_thread': (n_events // 8) / float(out1[3]), 'sum_w_pb': float(out[0]), 'n_pass': float(out[2]),
+            'sample': '%d events of the same Philox stream, gen/hoststep.cpp built with g++ -O3 -march=native -fopenmp '
+                      '(fp64; shared sub-currents, non-zero helicities only, colour-flow basis: the algorithm of the '
+                      'kernels, on CPU cores)' % n_events}
+
+
 def run_reference(args):
     rank = int(os.environ.get('RANK', '0'))
     if rank != 0:
@@ -401,6 +429,7 @@ def run_gpu(args):
 
     paper_ps = None if args.no_table else measure_paper_phase_space(torch, api, ctx, cfg, n, 5)
     cpu_base, _ = time_oracle(cfg, 4, 1)
+    cpu_gen = time_generated_host(cfg, {9: 1 << 14}.get(cfg, 1 << 19))
     s = acc[0] / acc[2]
     ds = (max(acc[1] / acc[2] - s * s, 0.0) / max(acc[2] - 1.0, 1.0)) ** 0.5
     line = {'metric': METRIC, 'value': value, 'unit': UNIT, 'n_gpus': world, 'steps': args.steps,
@@ -416,7 +445,7 @@ def run_gpu(args):
                        'pass_fraction': acc[3] / acc[2], 'sigma_pb': s, 'sigma_err_pb': ds},
             'clocks': clocks, 'e2e': e2e, 'gpu_launches': launches, 'roofline': roofline,
             'cpu_baseline': cpu_base, 'fma_peak_measured_tflops': peaks, 'per_config': per_config,
-            'paper_phase_space': paper_ps}
+            'paper_phase_space': paper_ps, 'cpu_generated_code': cpu_gen}
     print(json.dumps(line))
     ctx.close()
     if world > 1:

@@ -89,6 +89,10 @@ typedef struct {
   double alpha_em_inv;   /* 1/alpha */
   double alpha_s;        /* strong coupling, fixed */
   int ckm_diagonal;      /* must be 1 (only the diagonal CKM is implemented) */
+  int complex_mass;      /* 0: fixed widths in the propagator denominators only (default, reading A4).
+                            1: the paper's complex-mass option (Eq. 55-56): m_V^2 -> m_V^2 - i m_V
+                            Gamma_V (V = W, Z) also in the q q / m_V^2 term of the propagators and in the couplings
+                            g_W m_W, g_Z m_Z, 1/v; Eq. 56 fixes Gamma_W = mw gz / mz, the input gw is then ignored */
 } hg_params;
 
 /* Final-state cuts (Eq. 8-11; scope: SURVEY.md 8c-A11/A12).  A value <= 0 disables

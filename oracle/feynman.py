@@ -81,6 +81,8 @@ def anti(f):
 
 def mass_width(f, par):
     mk, wk = _F[f][2], _F[f][3]
+    if wk == 'gw':
+        return par[mk], sm.effective_widths(par)[0]      # Eq. 56 in the complex-mass option
     return (par[mk] if mk else 0.0), (par[wk] if wk else 0.0)
 
 
@@ -109,7 +111,12 @@ def build_vertices(par, names):
     """names: iterable of vertex keys, e.g. 'uug', 'udw', 'ggg', 'gggg', 'uua', 'eez' ..."""
     c = sm.couplings(par)
     gs = c['gs']
-    vev = 2.0 * par['mw'] / c['gw']
+    # complex-mass option (Eq. 55): m_V -> mu_V = sqrt(m_V^2 - i m_V Gamma_V) in the couplings
+    muw2, muz2 = sm.complex_masses(par)
+    cms = bool(par.get('complex_mass'))
+    mw_c = np.sqrt(muw2) if cms else par['mw']
+    mz_c = np.sqrt(muz2) if cms else par['mz']
+    vev = 2.0 * mw_c / c['gw']
     out = []
     for n in names:
         if n == 'ggg':
@@ -134,9 +141,9 @@ def build_vertices(par, names):
             y = -par['mt'] / vev
             out.append(Vertex('FFS', ('t~', 't', 'h'), row='t~', col='t', sca='h', gl=y, gr=y))
         elif n == 'wwh':
-            out.append(Vertex('VVS', ('w-', 'w+', 'h'), g=c['gw'] * par['mw']))
+            out.append(Vertex('VVS', ('w-', 'w+', 'h'), g=c['gw'] * mw_c))
         elif n == 'zzh':
-            out.append(Vertex('VVS', ('z', 'z', 'h'), g=c['gz'] * par['mz']))
+            out.append(Vertex('VVS', ('z', 'z', 'h'), g=c['gz'] * mz_c))
         elif n == 'wwhh':
             out.append(Vertex('VVSS', ('w-', 'w+', 'h', 'h'), g=0.5 * c['gw'] ** 2))
         elif n == 'zzhh':
@@ -421,7 +428,10 @@ def _propagate(field, K, cur, par):
     if s == 'V':
         if m == 0.0:
             return -1j * cur / den[:, None]
-        return -1j * (cur - K * (D.mdot(K, cur) / (m * m))[:, None]) / den[:, None]
+        m2 = m * m
+        if par.get('complex_mass'):       # Eq. 55 also in the q q / m_V^2 term
+            m2 = m * m - 1j * m * w
+        return -1j * (cur - K * (D.mdot(K, cur) / m2)[:, None]) / den[:, None]
     if not is_row(field):  # column spinor, fermion number flows with K
         num = D.slash(K) + m * D.ONE4
         return 1j * np.einsum('nab,nb->na', num, cur) / den[:, None]

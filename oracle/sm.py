@@ -12,7 +12,27 @@ HBARC2_PB = 0.3893793721e9  # (hbar c)^2 in pb GeV^2
 
 def default_params():
     return dict(mz=91.1876, mw=80.419, gz=2.441, gw=2.048, mt=174.3, gt=1.5, mb=0.0,
-                mh=125.0, gh=0.00407, alpha_em_inv=132.507, alpha_s=0.118)
+                mh=125.0, gh=0.00407, alpha_em_inv=132.507, alpha_s=0.118, complex_mass=0)
+
+
+def complex_masses(par):
+    """The paper's complex-mass option (Eq. 54-56; reading A4b in DESIGN.md): every m_V^2
+    (V = W, Z) in propagators AND couplings is replaced by mu_V^2 = m_V^2 - i m_V Gamma_V, with
+    mu_W^2 = (g_W^2 / g_Z^2) mu_Z^2 imposed (Eq. 56).  g_W^2 / g_Z^2 = cos^2 theta_W = m_W^2 / m_Z^2 is real here
+    (sw2 is derived from the real masses), so Eq. 56 fixes the W width: Gamma_W = m_W Gamma_Z / m_Z replaces the
+    input.  Returns (mu_W^2, mu_Z^2) as complex numbers; with complex_mass = 0 the real masses squared."""
+    if not par.get('complex_mass'):
+        return complex(par['mw'] ** 2), complex(par['mz'] ** 2)
+    muz2 = complex(par['mz'] ** 2, -par['mz'] * par['gz'])
+    muw2 = (par['mw'] ** 2 / par['mz'] ** 2) * muz2
+    return muw2, muz2
+
+
+def effective_widths(par):
+    """Widths in the propagator denominators: the inputs, or Eq. 56's W width in the complex-mass option."""
+    if not par.get('complex_mass'):
+        return par['gw'], par['gz']
+    return par['mw'] * par['gz'] / par['mz'], par['gz']
 
 
 # electric charge and weak isospin of the left-handed component
@@ -23,7 +43,11 @@ _T3 = {'u': 0.5, 'd': -0.5, 't': 0.5, 'b': -0.5, 'e-': -0.5, 'mu-': -0.5, 've': 
 
 def couplings(par):
     """Return a dict of real couplings derived from the inputs (tree-level relations)."""
-    sw2 = 1.0 - par['mw'] ** 2 / par['mz'] ** 2
+    ratio = par['mw'] ** 2 / par['mz'] ** 2
+    if isinstance(ratio, complex):      # complex masses of equal phase (analytic-continuation pin): the ratio is real
+        assert abs(ratio.imag) < 1e-14 * abs(ratio.real)
+        ratio = ratio.real
+    sw2 = 1.0 - ratio
     sw = math.sqrt(sw2)
     cw = math.sqrt(1.0 - sw2)
     e = math.sqrt(4.0 * math.pi / par['alpha_em_inv'])

@@ -25,7 +25,7 @@ BENCH_SYMBOLS = ('hg_set_profiling', 'hg_last_step_info', 'hg_measure_fma_peak')
 
 class hg_params(C.Structure):
     _fields_ = [(n, C.c_double) for n in ('mz', 'mw', 'gz', 'gw', 'mt', 'gt', 'mb', 'mh', 'gh', 'alpha_em_inv',
-                                          'alpha_s')] + [('ckm_diagonal', C.c_int)]
+                                          'alpha_s')] + [('ckm_diagonal', C.c_int), ('complex_mass', C.c_int)]
 
 
 class hg_cuts(C.Structure):

@@ -55,6 +55,8 @@ struct hg_ctx {
   const double* d_grid = nullptr;  // hg_set_grid: caller-owned [n_draws][grid_nb + 1]
   int grid_nb = 0;
   double* d_hist = nullptr;        // caller-owned [n_draws][grid_nb], or NULL
+  void* d_gstage = nullptr;          // global staging buffer of processes that stage in global memory (W + 4 jets)
+  size_t gstage_bytes = 0;
   double* d_hist_partial = nullptr;  // per-block histograms of one chunk
   size_t hist_partial_bytes = 0;
   cudaStream_t copy_stream = nullptr;   // H2D copies of hg_matrix_element_host
@@ -268,6 +270,20 @@ static void apply_sampling(const hg_ctx* ctx, PsConst& k) {
   }
 }
 
+// Global staging buffer of a process that stages in global memory (context-owned, grown on demand): sets *gblocks to
+// the size of its persistent grid (0 for every other process).
+static cudaError_t ensure_gstage(hg_ctx* ctx, const ProcVTable* vt, int precision, int* gblocks) {
+  size_t bytes = 0;
+  cudaError_t e = vt->gstage(precision, ctx->n_sm, gblocks, &bytes);
+  if (e != cudaSuccess || bytes <= ctx->gstage_bytes) return e;
+  if (ctx->d_gstage) cudaFree(ctx->d_gstage);
+  ctx->d_gstage = nullptr;
+  ctx->gstage_bytes = 0;
+  e = cudaMalloc(&ctx->d_gstage, bytes);
+  if (e == cudaSuccess) ctx->gstage_bytes = bytes;
+  return e;
+}
+
 static bool misaligned(const void* p, size_t al) { return ((uintptr_t)p % al) != 0; }
 
 static bool finite_pos(double x) { return isfinite(x) && x > 0.0; }
@@ -318,6 +334,7 @@ void hg_destroy(hg_ctx* ctx) {
   if (ctx->d_stage) cudaFree(ctx->d_stage);
   if (ctx->d_scratch) cudaFree(ctx->d_scratch);
   if (ctx->d_hist_partial) cudaFree(ctx->d_hist_partial);
+  if (ctx->d_gstage) cudaFree(ctx->d_gstage);
   for (cudaEvent_t ev : ctx->ev) cudaEventDestroy(ev);
   for (int i = 0; i < 2; ++i) {
     if (ctx->ev_h2d[i]) cudaEventDestroy(ctx->ev_h2d[i]);
@@ -358,6 +375,8 @@ int hg_set_params(hg_ctx* ctx, const hg_params* par, const hg_cuts* cuts) {
   if (par->mb != 0.0) return fail(ctx, HG_EINVAL, "hg_set_params: only mb = 0 is generated (BASELINE.json)");
   if (!(par->mw < par->mz)) return fail(ctx, HG_EINVAL, "hg_set_params: need mw < mz (sw2 = 1 - mw^2/mz^2)");
   if (par->ckm_diagonal != 1) return fail(ctx, HG_EINVAL, "hg_set_params: only the diagonal CKM is implemented");
+  if (par->complex_mass != 0 && par->complex_mass != 1)
+    return fail(ctx, HG_EINVAL, "hg_set_params: complex_mass must be 0 or 1");
   if (cuts) {
     const double v[4] = {cuts->pt_jet_min, cuts->eta_jet_max, cuts->eta_lep_max, cuts->dr_jj_min};
     for (int i = 0; i < 4; ++i)
@@ -461,7 +480,10 @@ int hg_matrix_element(hg_ctx* ctx, int process, int precision, int64_t n, const 
   if (((uintptr_t)d_p % al) || ((uintptr_t)d_me2 % al))
     return fail(ctx, HG_EINVAL, "hg_matrix_element: misaligned pointer");
   HG_ON_DEVICE(ctx, "hg_matrix_element");
-  cudaError_t e = vt->me(precision, n, d_p, d_me2, ctx->coup, (cudaStream_t)cuda_stream);
+  int gblocks = 0;
+  cudaError_t e = ensure_gstage(ctx, vt, precision, &gblocks);
+  if (e != cudaSuccess) return fail_cuda(ctx, e, "hg_matrix_element: global staging buffer");
+  e = vt->me(precision, n, d_p, d_me2, ctx->coup, ctx->d_gstage, gblocks, (cudaStream_t)cuda_stream);
   if (e != cudaSuccess) return fail_cuda(ctx, e, "hg_matrix_element");
   return HG_OK;
 }
@@ -492,7 +514,9 @@ int hg_matrix_element_host(hg_ctx* ctx, int process, int precision, int64_t n, c
     if (e != cudaSuccess) return fail_cuda(ctx, e, "hg_matrix_element_host: cudaMalloc");
     ctx->stage_bytes = 2 * buf_bytes;
   }
-  cudaError_t e = cudaSuccess;
+  int gblocks = 0;
+  cudaError_t e = ensure_gstage(ctx, vt, precision, &gblocks);
+  if (e != cudaSuccess) return fail_cuda(ctx, e, "hg_matrix_element_host: global staging buffer");
   if (!ctx->copy_stream) {
     e = cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking);
     for (int i = 0; i < 2 && e == cudaSuccess; ++i) {
@@ -517,7 +541,7 @@ int hg_matrix_element_host(hg_ctx* ctx, int process, int precision, int64_t n, c
                             el * (size_t)m, rows, cudaMemcpyHostToDevice, ctx->copy_stream);
     if (e == cudaSuccess) e = cudaEventRecord(ctx->ev_h2d[b], ctx->copy_stream);
     if (e == cudaSuccess) e = cudaStreamWaitEvent(s, ctx->ev_h2d[b], 0);
-    if (e == cudaSuccess) e = vt->me(precision, m, d_in, d_out, ctx->coup, s);
+    if (e == cudaSuccess) e = vt->me(precision, m, d_in, d_out, ctx->coup, ctx->d_gstage, gblocks, s);
     if (e == cudaSuccess)
       e = cudaMemcpyAsync((char*)h_me2 + el * (size_t)off, d_out, el * (size_t)m, cudaMemcpyDeviceToHost, s);
     if (e == cudaSuccess) e = cudaEventRecord(ctx->ev_free[b], s);
@@ -594,6 +618,10 @@ int hg_integrate_step(hg_ctx* ctx, int process, int precision, uint64_t seed, ui
   if (per_sm < 1) per_sm = 1;
   int nblocks = ctx->n_sm * per_sm;  // persistent grid: a whole number of resident waves
   if (nblocks > kMaxPartialBlocks) nblocks = kMaxPartialBlocks;
+  int gblocks = 0;
+  e = ensure_gstage(ctx, vt, precision, &gblocks);
+  if (e != cudaSuccess) return fail_cuda(ctx, e, "hg_integrate_step: global staging buffer");
+  if (gblocks > 0 && nblocks > gblocks) nblocks = gblocks;
   const int64_t need = (n + kIntThreads - 1) / kIntThreads;
   if (need < nblocks) nblocks = (int)need;
   const int64_t chunk = n < kIntChunk ? n : kIntChunk;
@@ -635,7 +663,7 @@ int hg_integrate_step(hg_ctx* ctx, int process, int precision, uint64_t seed, ui
     ev = ctx->ev.data();
   }
   e = vt->integrate(precision, n, k, seed, first_event, ctx->coup, wscale, ctx->d_partials, nblocks, ctx->d_scratch,
-                    chunk, ev, hist ? &ga : nullptr, s);
+                    chunk, ev, hist ? &ga : nullptr, ctx->d_gstage, s);
   if (e != cudaSuccess) return fail_cuda(ctx, e, "hg_integrate_step");
   ctx->n_launches = (per_event ? (hist ? 5 : 3) * nchunks : 1) + 1;
   rc = finish(ctx, nblocks, n, acc, s, "hg_integrate_step");  // synchronises the stream

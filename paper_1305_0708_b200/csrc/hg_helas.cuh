@@ -406,8 +406,8 @@ HG_HD Vc<T> ffv_current(const Sp<T>& fi, const Sp<T>& fo, T gL, T gR) {
 
 // Vector propagator applied to a bare current: massless / Feynman gauge d J; massive / unitary gauge
 // d (J - q (q.J) / m^2)   (reading A4: real m^2 in the q q / m^2 term).
-template <bool UNITARY, class T, class D>
-HG_HD Vc<T> vprop(const Vc<T>& j, const Mom<T>& q, T rm2, D d) {
+template <bool UNITARY, class T, class D, class R>
+HG_HD Vc<T> vprop(const Vc<T>& j, const Mom<T>& q, R rm2, D d) {
   Vc<T> w;
   if (UNITARY) {
     cx<T> s = rm2 * vdot(q, j);
@@ -422,8 +422,8 @@ HG_HD Vc<T> vprop(const Vc<T>& j, const Mom<T>& q, T rm2, D d) {
 }
 
 // jioxxx: off-shell vector from a fermion pair.  q = total momentum, rm2 = 1/m^2.
-template <int MI, int MO, int G, bool UNITARY, class T, class D>
-HG_HD Vc<T> jioxxx(const Sp<T>& fi, const Sp<T>& fo, T gL, T gR, const Mom<T>& q, T rm2, D d) {
+template <int MI, int MO, int G, bool UNITARY, class T, class D, class R>
+HG_HD Vc<T> jioxxx(const Sp<T>& fi, const Sp<T>& fo, T gL, T gR, const Mom<T>& q, R rm2, D d) {
   return vprop<UNITARY>(ffv_current<MI, MO, G>(fi, fo, gL, gR), q, rm2, d);
 }
 
@@ -448,8 +448,8 @@ HG_HD cx<T> vvvxxx(const Vc<T>& v1, const Vc<T>& v2, const Vc<T>& v3, T g, const
 }
 // jvvxxx: off-shell vector from two vectors; k3 = -(k1+k2).
 //   J = g [ (v1.v2)(k1-k2) + v2 ((2 k2 + k1).v1) - v1 ((2 k1 + k2).v2) ],  result = vprop(J, k1+k2)
-template <bool UNITARY, class T, class D>
-HG_HD Vc<T> jvvxxx(const Vc<T>& v1, const Vc<T>& v2, T g, const Mom<T>& k1, const Mom<T>& k2, T rm2, D d) {
+template <bool UNITARY, class T, class D, class R>
+HG_HD Vc<T> jvvxxx(const Vc<T>& v1, const Vc<T>& v2, T g, const Mom<T>& k1, const Mom<T>& k2, R rm2, D d) {
   cx<T> d12 = g * vdot(v1, v2);
   cx<T> a = g * vdot(k2 + k2 + k1, v1);
   cx<T> b = g * vdot(k1 + k1 + k2, v2);
@@ -582,24 +582,24 @@ HG_HD Vc<T> jggg_bare(const Vc<T>& v1, const Vc<T>& v2, const Vc<T>& v3, T g2) {
 // L = psibar (gL PL + gR PR) psi S.  In the chiral basis PL keeps column slots A and pairs them with ROW slots A
 // (psibar = psi^dagger gamma^0 has the conjugate RIGHT part in its slots A), PR pairs slots B with B.
 // iosxxx: amplitude (C.4.1)
-template <int MI, int MO, int G, class T>
-HG_HD cx<T> iosxxx(const Sp<T>& fi, const Sp<T>& fo, cx<T> s, T gL, T gR) {
+template <int MI, int MO, int G, class T, class C_>
+HG_HD cx<T> iosxxx(const Sp<T>& fi, const Sp<T>& fo, cx<T> s, C_ gL, C_ gR) {
   cx<T> r = czero<T>();
   if ((MI & SLOT_A) && (MO & SLOT_A) && (G & CPL_L)) r = gL * cfma(fo.c[1], fi.c[1], fo.c[0] * fi.c[0]);
   if ((MI & SLOT_B) && (MO & SLOT_B) && (G & CPL_R)) r = r + gR * cfma(fo.c[3], fi.c[3], fo.c[2] * fi.c[2]);
   return s * r;
 }
 // hioxxx: off-shell scalar from a fermion pair (C.4.4); d = -1/(q^2 - m^2 + i m Gamma)
-template <int MI, int MO, int G, class T, class D>
-HG_HD cx<T> hioxxx(const Sp<T>& fi, const Sp<T>& fo, T gL, T gR, D d) {
+template <int MI, int MO, int G, class T, class D, class C_>
+HG_HD cx<T> hioxxx(const Sp<T>& fi, const Sp<T>& fo, C_ gL, C_ gR, D d) {
   cx<T> r = czero<T>();
   if ((MI & SLOT_A) && (MO & SLOT_A) && (G & CPL_L)) r = gL * cfma(fo.c[1], fi.c[1], fo.c[0] * fi.c[0]);
   if ((MI & SLOT_B) && (MO & SLOT_B) && (G & CPL_R)) r = r + gR * cfma(fo.c[3], fi.c[3], fo.c[2] * fi.c[2]);
   return d * r;
 }
 // fsixxx: off-shell flowing-IN fermion  d (qslash + m) (gL PL + gR PR) |fi> S   (C.4.2)
-template <int MI, int G, bool MASSIVE, class T, class D>
-HG_HD Sp<T> fsixxx(const Sp<T>& fi, cx<T> s, T gL, T gR, const Mom<T>& q, T m, D d) {
+template <int MI, int G, bool MASSIVE, class T, class D, class C_>
+HG_HD Sp<T> fsixxx(const Sp<T>& fi, cx<T> s, C_ gL, C_ gR, const Mom<T>& q, T m, D d) {
   constexpr bool L = (MI & SLOT_A) && (G & CPL_L);  // w_A = gL S fi_A
   constexpr bool R = (MI & SLOT_B) && (G & CPL_R);  // w_B = gR S fi_B
   cx<T> wA0 = czero<T>(), wA1 = czero<T>(), wB0 = czero<T>(), wB1 = czero<T>();
@@ -639,8 +639,8 @@ HG_HD Sp<T> fsixxx(const Sp<T>& fi, cx<T> s, T gL, T gR, const Mom<T>& q, T m, D
   return f;
 }
 // fsoxxx: off-shell flowing-OUT fermion  d <fo| (gL PL + gR PR) S (qslash + m)   (C.4.3)
-template <int MO, int G, bool MASSIVE, class T, class D>
-HG_HD Sp<T> fsoxxx(const Sp<T>& fo, cx<T> s, T gL, T gR, const Mom<T>& q, T m, D d) {
+template <int MO, int G, bool MASSIVE, class T, class D, class C_>
+HG_HD Sp<T> fsoxxx(const Sp<T>& fo, cx<T> s, C_ gL, C_ gR, const Mom<T>& q, T m, D d) {
   constexpr bool L = (MO & SLOT_A) && (G & CPL_L);  // w_A = gL S fo_A
   constexpr bool R = (MO & SLOT_B) && (G & CPL_R);  // w_B = gR S fo_B
   cx<T> wA0 = czero<T>(), wA1 = czero<T>(), wB0 = czero<T>(), wB1 = czero<T>();
@@ -683,41 +683,41 @@ HG_HD Sp<T> fsoxxx(const Sp<T>& fo, cx<T> s, T gL, T gR, const Mom<T>& q, T m, D
 // =============================================================================== VVS, VVSS, SSS (Eq. 50-52)
 // L_VVS = g (V1.V2) S, L_VVSS = g (V1.V2) S3 S4, L_SSS = g S1 S2 S3 (C.7-C.9); g is the
 // coefficient of the Feynman rule (W W H: gW mW, Z Z H: gZ mZ, W W H H: gW^2/2, Z Z H H: gZ^2/2, H H H: -3 mH^2/v).
-template <class T>
-HG_HD cx<T> vvsxxx(const Vc<T>& v1, const Vc<T>& v2, cx<T> s, T g) {
+template <class T, class C_>
+HG_HD cx<T> vvsxxx(const Vc<T>& v1, const Vc<T>& v2, cx<T> s, C_ g) {
   return g * (s * vdot(v1, v2));
 }
 // jvsxxx: off-shell vector from a vector and a scalar
-template <bool UNITARY, class T, class D>
-HG_HD Vc<T> jvsxxx(const Vc<T>& v, cx<T> s, T g, const Mom<T>& q, T rm2, D d) {
+template <bool UNITARY, class T, class D, class R, class C_>
+HG_HD Vc<T> jvsxxx(const Vc<T>& v, cx<T> s, C_ g, const Mom<T>& q, R rm2, D d) {
   const cx<T> gs = g * s;
   Vc<T> j;
   for (int i = 0; i < 4; ++i) j.c[i] = gs * v.c[i];
   return vprop<UNITARY>(j, q, rm2, d);
 }
 // hvvxxx: off-shell scalar from two vectors; d = -1/(q^2 - m^2 + i m Gamma)
-template <class T, class D>
-HG_HD cx<T> hvvxxx(const Vc<T>& v1, const Vc<T>& v2, T g, D d) {
+template <class T, class D, class C_>
+HG_HD cx<T> hvvxxx(const Vc<T>& v1, const Vc<T>& v2, C_ g, D d) {
   return d * (g * vdot(v1, v2));
 }
 template <class T>
 HG_HD cx<T> vvssxx(const Vc<T>& v1, const Vc<T>& v2, cx<T> s3, cx<T> s4, T g) {
   return g * (s3 * s4 * vdot(v1, v2));
 }
-template <bool UNITARY, class T, class D>
-HG_HD Vc<T> jvssxx(const Vc<T>& v, cx<T> s3, cx<T> s4, T g, const Mom<T>& q, T rm2, D d) {
+template <bool UNITARY, class T, class D, class R>
+HG_HD Vc<T> jvssxx(const Vc<T>& v, cx<T> s3, cx<T> s4, T g, const Mom<T>& q, R rm2, D d) {
   return jvsxxx<UNITARY>(v, s3 * s4, g, q, rm2, d);
 }
 template <class T, class D>
 HG_HD cx<T> hvvsxx(const Vc<T>& v1, const Vc<T>& v2, cx<T> s, T g, D d) {
   return d * (g * (s * vdot(v1, v2)));
 }
-template <class T>
-HG_HD cx<T> sssxxx(cx<T> s1, cx<T> s2, cx<T> s3, T g) {
+template <class T, class C_>
+HG_HD cx<T> sssxxx(cx<T> s1, cx<T> s2, cx<T> s3, C_ g) {
   return g * (s1 * s2 * s3);
 }
-template <class T, class D>
-HG_HD cx<T> hssxxx(cx<T> s1, cx<T> s2, T g, D d) {
+template <class T, class D, class C_>
+HG_HD cx<T> hssxxx(cx<T> s1, cx<T> s2, C_ g, D d) {
   return d * (g * (s1 * s2));
 }
 

@@ -22,6 +22,7 @@ inline void default_params(hg_params* p) {
   p->alpha_em_inv = 132.507;
   p->alpha_s = 0.118;
   p->ckm_diagonal = 1;
+  p->complex_mass = 0;
 }
 
 // BASELINE.json configs; scope readings SURVEY.md 8c-A11/A12.

@@ -31,7 +31,9 @@ struct GridAcc {
 struct ProcVTable {
   hg_process_info_t info;
   // hg_matrix_element: p [n_ext][4][n] -> me2 [n]
-  cudaError_t (*me)(int prec, int64_t n, const void* d_p, void* d_me2, const Coup<double>& c, cudaStream_t s);
+  // d_gstage / gblocks: global staging buffer and grid of processes that stage in global memory (gstage below)
+  cudaError_t (*me)(int prec, int64_t n, const void* d_p, void* d_me2, const Coup<double>& c, void* d_gstage,
+                    int gblocks, cudaStream_t s);
   // hg_gen_phase_space
   cudaError_t (*ps)(int prec, int64_t n, const PsConst& k, uint64_t seed, uint64_t first, void* d_p,
                     void* d_wps, uint8_t* d_pass, cudaStream_t s);
@@ -43,7 +45,8 @@ struct ProcVTable {
   // ga (or NULL): adaptive-grid step, histograms accumulated after each chunk.
   cudaError_t (*integrate)(int prec, int64_t n, const PsConst& k, uint64_t seed, uint64_t first,
                            const Coup<double>& c, double wscale, double* d_partials, int nblocks,
-                           void* d_scratch, int64_t chunk, cudaEvent_t* ev, const GridAcc* ga, cudaStream_t s);
+                           void* d_scratch, int64_t chunk, cudaEvent_t* ev, const GridAcc* ga, void* d_gstage,
+                           cudaStream_t s);
   // resident blocks per SM of the kernel that evaluates the matrix element in the step (occupancy query); split:
   // the split step is forced (adaptive-grid steps run every process as separate kernels)
   cudaError_t (*int_blocks_per_sm)(int prec, bool split, int* out);
@@ -51,6 +54,8 @@ struct ProcVTable {
   size_t (*scratch_bytes)(int prec, int64_t chunk, bool grid);
   bool (*split_step)();
   bool (*has_hadronic)();   // the paper's hadronic phase space is implemented for this process
+  // global staging buffer (W + 4 jets): blocks of the persistent grid and bytes; 0 / 0 if staged in shared memory
+  cudaError_t (*gstage)(int prec, int n_sm, int* blocks, size_t* bytes);
 };
 
 extern const ProcVTable hg_proc_1, hg_proc_2, hg_proc_3, hg_proc_4, hg_proc_5, hg_proc_6, hg_proc_7, hg_proc_8, hg_proc_9,

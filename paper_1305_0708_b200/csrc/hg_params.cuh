@@ -18,6 +18,9 @@ struct Coup {
   T gzuL, gzuR, gzdL, gzdR, gzlL, gzlR, gznL;  // Z: -g_Z (T3 - Q sw2),  +g_Z Q sw2
   // gauge and Higgs self couplings (library vertices; Table 16, Eq. 39, 50-52)
   T gwwa, gwwz, gtth, gwwh, gzzh, gwwhh, gzzhh, ghhh;
+  // imaginary parts of the couplings that contain m_W, m_Z (complex-mass option, Eq. 55-56 PAPER.md:1066-1073;
+  // zero otherwise) and the flag itself (1 or 0): the q q / m_V^2 term then uses m_V^2 - i m_V Gamma_V
+  T gtth_i, gwwh_i, gzzh_i, ghhh_i, cms;
   // masses and widths
   T mz, wz, mw, ww, mt, wt, mh, wh;
 };

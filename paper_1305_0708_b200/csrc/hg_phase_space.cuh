@@ -18,16 +18,39 @@ namespace hg {
 
 #define HG_TWO_PI 6.283185307179586476925286766559
 
+// The fp64 transcendental functions of the phase space are CALLED, not inlined: one copy each of log, sincospi,
+// asinh and atan2 instead of five or six.  The flat W + 3 jets phase-space kernel executed 4,660 instructions per
+// event with 3.3 instruction-fetch stalls per issue (profiles/r02_notes.md): its straight-line code did not fit the
+// instruction cache.
+#if defined(__CUDACC__)
+#define HG_CALL static __host__ __device__ __noinline__
+#else
+#define HG_CALL inline
+#endif
+HG_CALL double hlog(double x) { return log(x); }
+HG_CALL double hasinh(double x) { return asinh(x); }
+HG_CALL double hatan2(double y, double x) { return atan2(y, x); }
+
 // sin, cos of 2 pi u.  On the device sincospi(2u): exact argument reduction, so no call to the Payne-Hanek slow path
 // of sincos() is left in the fused kernels (a real CALL inside the W+3 jets fp64 kernel made ptxas fall back to an
 // all-on-stack allocation, profiles/r01_notes.md).
-HG_HD void hsincos2pi(double u, double& s, double& c) {
+struct SinCos {
+  double s, c;
+};
+HG_CALL SinCos hsincos2pi_call(double u) {
+  SinCos r;
 #if defined(__CUDA_ARCH__)
-  sincospi(2.0 * u, &s, &c);
+  sincospi(2.0 * u, &r.s, &r.c);
 #else
-  s = sin(HG_TWO_PI * u);
-  c = cos(HG_TWO_PI * u);
+  r.s = sin(HG_TWO_PI * u);
+  r.c = cos(HG_TWO_PI * u);
 #endif
+  return r;
+}
+HG_HD void hsincos2pi(double u, double& s, double& c) {
+  const SinCos r = hsincos2pi_call(u);   // returned in registers: no stack traffic for the two results
+  s = r.s;
+  c = r.c;
 }
 
 // Constants of one hg_gen_phase_space / hg_integrate_step call, prepared on the host.
@@ -91,7 +114,7 @@ HG_HD void rambo_massless(const double* u, double rs, Mom<double>* p) {
   Mom<double> Q = mkmom<double>(0, 0, 0, 0);
 #pragma unroll
   for (int i = 0; i < N; ++i) {
-    p[i] = iso(u[4 * i], u[4 * i + 1], -log(u[4 * i + 2] * u[4 * i + 3]));
+    p[i] = iso(u[4 * i], u[4 * i + 1], -hlog(u[4 * i + 2] * u[4 * i + 3]));
     Q = Q + p[i];
   }
   const double rM = 1.0 / sqrt(mdot(Q, Q));
@@ -408,10 +431,10 @@ HG_HD double gen_had_ttxg_dilep(const PsConst& k, uint64_t seed, uint64_t event,
 
 // ---------------------------------------------------------------- cuts (Eq. 8-11)
 HG_HD double pt_of(const Mom<double>& p) { return sqrt(p.x * p.x + p.y * p.y); }
-HG_HD double eta_of(const Mom<double>& p) { return asinh(p.z / pt_of(p)); }
+HG_HD double eta_of(const Mom<double>& p) { return hasinh(p.z / pt_of(p)); }
 HG_HD double delta_r(const Mom<double>& a, const Mom<double>& b) {  // Eq. 9b
   const double pi = 0.5 * HG_TWO_PI;
-  double dphi = atan2(a.y, a.x) - atan2(b.y, b.x);
+  double dphi = hatan2(a.y, a.x) - hatan2(b.y, b.x);
   if (dphi > pi) dphi -= HG_TWO_PI;
   if (dphi < -pi) dphi += HG_TWO_PI;
   const double deta = eta_of(a) - eta_of(b);

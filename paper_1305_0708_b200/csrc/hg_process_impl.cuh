@@ -29,9 +29,11 @@ namespace hg {
 constexpr int kSmemPerSM = 227 * 1024;
 template <class P>
 constexpr int kSplit = P::n_stage > 0 ? 2 : 1;
+constexpr int kGlobalStageThreads = 256;   // global staging area: 4 pairs per block, limited by registers
 template <class P, class T>
 constexpr int stage_threads(int want) {
   if (P::n_stage == 0) return want;
+  if (P::stage_global) return kGlobalStageThreads;
   // 32-event groups that fit on an SM, leaving 3 KB for the kernels' static shared memory
   const int groups = (kSmemPerSM - 3072) / (P::n_stage * (int)sizeof(T) * 32);
   // 2, 4 or 6 pairs = 4, 8 or 12 warps: a multiple of the 4 schedulers (6 and 10 warps measured slower than 4 and 8)
@@ -40,7 +42,7 @@ constexpr int stage_threads(int want) {
 }
 template <class P, class T, int THREADS>
 constexpr size_t stage_bytes() {
-  return (size_t)P::n_stage * sizeof(T) * (THREADS / kSplit<P>);
+  return P::stage_global ? 0 : (size_t)P::n_stage * sizeof(T) * (THREADS / kSplit<P>);
 }
 // index of this thread's event within the block, and whether this thread owns the event's result
 template <class P>
@@ -56,16 +58,23 @@ __device__ __forceinline__ bool ev_owner() {
 
 // me2 of one event.  Staged: the staging area of the event is shared memory laid out [slot][event] (hg_stage.cuh);
 // every thread of the block must call; the total is returned to the owner thread of the pair.
+// gstage: global staging buffer of gridDim.x * EPB columns (P::stage_global), else unused.
 template <class P, class T, int THREADS>
-__device__ __forceinline__ T me2_event(const Mom<T>* q, const Coup<T>& c) {
+__device__ __forceinline__ T me2_event(const Mom<T>* q, const Coup<T>& c, T* gstage) {
   if constexpr (P::n_stage > 0) {
     constexpr int EPB = THREADS / 2;
     extern __shared__ __align__(16) unsigned char hg_stage_smem[];
     __shared__ T comb[EPB];
     const int ev = ev_local<P>();
     const int half = (threadIdx.x >> 5) & 1;
-    const SmemStage<T, EPB> st{reinterpret_cast<T*>(hg_stage_smem) + ev, half};
-    T r = P::template me2<T>(q, c, st);
+    T r;
+    if constexpr (P::stage_global) {
+      const GmemStage<T> st{gstage + (int64_t)blockIdx.x * EPB + ev, (int64_t)gridDim.x * EPB, half};
+      r = P::template me2<T>(q, c, st);
+    } else {
+      const SmemStage<T, EPB> st{reinterpret_cast<T*>(hg_stage_smem) + ev, half};
+      r = P::template me2<T>(q, c, st);
+    }
     if (half) comb[ev] = r;
     __syncthreads();
     if (!half) r += comb[ev];
@@ -76,18 +85,22 @@ __device__ __forceinline__ T me2_event(const Mom<T>* q, const Coup<T>& c) {
   }
 }
 
+// Grid: one block per EPB events, or (P::stage_global) a persistent grid that strides over the batches, each block
+// keeping its EPB columns of the global staging buffer.
 template <class P, class T, int THREADS>
 __global__ void __launch_bounds__(THREADS) me_kernel(const T* __restrict__ p, T* __restrict__ me2, int64_t n,
-                                                     const Coup<T> c) {
+                                                     const Coup<T> c, T* gstage) {
   constexpr int EPB = THREADS / kSplit<P>;
-  const int64_t e0 = (int64_t)blockIdx.x * EPB + ev_local<P>();
-  const int64_t e = e0 < n ? e0 : n - 1;  // no early exit: a staged me2 holds block-wide rendezvous
-  Mom<T> q[P::n_ext];
+  for (int64_t base = (int64_t)blockIdx.x * EPB; base < n; base += (int64_t)gridDim.x * EPB) {   // block-uniform
+    const int64_t e0 = base + ev_local<P>();
+    const int64_t e = e0 < n ? e0 : n - 1;  // no early exit: a staged me2 holds block-wide rendezvous
+    Mom<T> q[P::n_ext];
 #pragma unroll
-  for (int l = 0; l < P::n_ext; ++l)
-    q[l] = mkmom<T>(p[(l * 4 + 0) * n + e], p[(l * 4 + 1) * n + e], p[(l * 4 + 2) * n + e], p[(l * 4 + 3) * n + e]);
-  const T r = me2_event<P, T, THREADS>(q, c);
-  if (e0 < n && ev_owner<P>()) me2[e0] = r;
+    for (int l = 0; l < P::n_ext; ++l)
+      q[l] = mkmom<T>(p[(l * 4 + 0) * n + e], p[(l * 4 + 1) * n + e], p[(l * 4 + 2) * n + e], p[(l * 4 + 3) * n + e]);
+    const T r = me2_event<P, T, THREADS>(q, c, gstage);
+    if (e0 < n && ev_owner<P>()) me2[e0] = r;
+  }
 }
 
 // BEAMS = true: all n_ext legs are written (hg_gen_phase_space).  BEAMS = false (chunk buffer of the split step): only
@@ -174,7 +187,7 @@ __global__ void __launch_bounds__(THREADS) integrate_kernel(const PsConst k, uin
       Mom<T> qt[P::n_ext];
 #pragma unroll
       for (int l = 0; l < P::n_ext; ++l) qt[l] = mkmom<T>(T(q[l].e), T(q[l].x), T(q[l].y), T(q[l].z));
-      const double w = (double)me2_event<P, T, THREADS>(qt, c) * wps * wscale;
+      const double w = (double)me2_event<P, T, THREADS>(qt, c, nullptr) * wps * wscale;
       sw += w;
       sw2 += w * w;
       np += 1.0;
@@ -234,7 +247,8 @@ __global__ void __launch_bounds__(THREADS) me_acc_kernel(const T* __restrict__ p
                                                          const int* __restrict__ idx, const int* __restrict__ cnt,
                                                          int64_t n, int64_t range, const Coup<T> c, double wscale,
                                                          double ebeam, const double* __restrict__ beams, int add,
-                                                         double* __restrict__ partials, double* __restrict__ wout) {
+                                                         double* __restrict__ partials, double* __restrict__ wout,
+                                                         T* gstage) {
   constexpr int EPB = THREADS / kSplit<P>;
   double sw = 0.0, sw2 = 0.0, np = 0.0;
   const int m = cnt[blockIdx.x];                    // passing events of this block's range, block-uniform
@@ -251,7 +265,7 @@ __global__ void __launch_bounds__(THREADS) me_acc_kernel(const T* __restrict__ p
     for (int l = 2; l < P::n_ext; ++l)
       q[l] = mkmom<T>(p[((l - 2) * 4 + 0) * n + e], p[((l - 2) * 4 + 1) * n + e], p[((l - 2) * 4 + 2) * n + e],
                       p[((l - 2) * 4 + 3) * n + e]);
-    const double w = (double)me2_event<P, T, THREADS>(q, c) * wps[e] * wscale;
+    const double w = (double)me2_event<P, T, THREADS>(q, c, gstage) * wps[e] * wscale;
     if (ok && ev_owner<P>()) {
       sw += w;
       sw2 += w * w;
@@ -284,20 +298,45 @@ struct Launch {
     if (bytes <= 48 * 1024) return cudaSuccess;
     return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
   }
+  // gblocks: blocks of the persistent grid, d_gstage: global staging buffer (P::stage_global only, gstage())
   template <class T>
-  static cudaError_t me_t(int64_t n, const void* d_p, void* d_me2, const Coup<T>& c, cudaStream_t s) {
+  static cudaError_t me_t(int64_t n, const void* d_p, void* d_me2, const Coup<T>& c, void* d_gstage, int gblocks,
+                          cudaStream_t s) {
     constexpr int TH = me_thr<T>();
     constexpr size_t smem = stage_bytes<P, T, TH>();
     cudaError_t err = allow_smem(me_kernel<P, T, TH>, smem);
     if (err != cudaSuccess) return err;
     constexpr int EPB = TH / kSplit<P>;
-    const unsigned grid = (unsigned)((n + EPB - 1) / EPB);
-    me_kernel<P, T, TH><<<grid, TH, smem, s>>>((const T*)d_p, (T*)d_me2, n, c);
+    unsigned grid = (unsigned)((n + EPB - 1) / EPB);
+    if (P::stage_global && grid > (unsigned)gblocks) grid = (unsigned)gblocks;
+    me_kernel<P, T, TH><<<grid, TH, smem, s>>>((const T*)d_p, (T*)d_me2, n, c, (T*)d_gstage);
     return cudaGetLastError();
   }
-  static cudaError_t me(int prec, int64_t n, const void* d_p, void* d_me2, const Coup<double>& c, cudaStream_t s) {
-    if (prec == HG_F64) return me_t<double>(n, d_p, d_me2, c, s);
-    return me_t<float>(n, d_p, d_me2, coup_cast<float>(c), s);
+  static cudaError_t me(int prec, int64_t n, const void* d_p, void* d_me2, const Coup<double>& c, void* d_gstage,
+                        int gblocks, cudaStream_t s) {
+    if (prec == HG_F64) return me_t<double>(n, d_p, d_me2, c, d_gstage, gblocks, s);
+    return me_t<float>(n, d_p, d_me2, coup_cast<float>(c), d_gstage, gblocks, s);
+  }
+  // Global staging buffer: resident blocks per SM of the two kernels that evaluate me2 (the smaller one) and the
+  // bytes of a buffer for n_sm * that many blocks; 0 blocks / 0 bytes for processes that stage in shared memory.
+  template <class T>
+  static cudaError_t gstage_t(int n_sm, int* blocks, size_t* bytes) {
+    *blocks = 0;
+    *bytes = 0;
+    if constexpr (P::n_stage > 0 && P::stage_global) {
+      constexpr int TH = me_thr<T>();
+      int a = 0, b = 0;
+      cudaError_t err = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&a, me_kernel<P, T, TH>, TH, 0);
+      if (err == cudaSuccess) err = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&b, me_acc_kernel<P, T, TH>, TH, 0);
+      if (err != cudaSuccess) return err;
+      const int per_sm = a < b ? a : b;
+      *blocks = n_sm * (per_sm < 1 ? 1 : per_sm);
+      *bytes = (size_t)*blocks * (TH / 2) * P::n_stage * sizeof(T);
+    }
+    return cudaSuccess;
+  }
+  static cudaError_t gstage(int prec, int n_sm, int* blocks, size_t* bytes) {
+    return prec == HG_F64 ? gstage_t<double>(n_sm, blocks, bytes) : gstage_t<float>(n_sm, blocks, bytes);
   }
   // the four (grid, hadronic) variants of the phase-space kernel are separate instantiations
   template <class T, class W, bool BEAMS>
@@ -350,7 +389,7 @@ struct Launch {
   template <class T>
   static cudaError_t integrate_t(int64_t n, const PsConst& k, uint64_t seed, uint64_t first, const Coup<T>& c,
                                  double wscale, double* d_partials, int nblocks, void* d_scratch, int64_t chunk,
-                                 cudaEvent_t* ev, const GridAcc* ga, cudaStream_t s) {
+                                 cudaEvent_t* ev, const GridAcc* ga, void* d_gstage, cudaStream_t s) {
     constexpr int TH = int_thr<T>();
     constexpr size_t smem = stage_bytes<P, T, TH>();
     if constexpr (!P::split_step) {
@@ -383,7 +422,7 @@ struct Launch {
       compact_kernel<<<nblocks, 256, 0, s>>>(d_ok, m, range, d_idx, d_cnt);
       if (e3) cudaEventRecord(e3[1], s);
       me_acc_kernel<P, T, TH><<<nblocks, TH, smem, s>>>(d_p, d_w, d_idx, d_cnt, m, range, c, wscale, 0.5 * k.rs,
-                                                        d_beams, off > 0 ? 1 : 0, d_partials, d_wout);
+                                                        d_beams, off > 0 ? 1 : 0, d_partials, d_wout, (T*)d_gstage);
       if (e3) cudaEventRecord(e3[2], s);
       if (ga) {
         err = ga->launch(d_bins, d_wout, d_idx, d_cnt, m, range, nblocks, P::n_draws, s);
@@ -394,11 +433,13 @@ struct Launch {
   }
   static cudaError_t integrate(int prec, int64_t n, const PsConst& k, uint64_t seed, uint64_t first,
                                const Coup<double>& c, double wscale, double* d_partials, int nblocks,
-                               void* d_scratch, int64_t chunk, cudaEvent_t* ev, const GridAcc* ga, cudaStream_t s) {
+                               void* d_scratch, int64_t chunk, cudaEvent_t* ev, const GridAcc* ga, void* d_gstage,
+                               cudaStream_t s) {
     if (prec == HG_F64)
-      return integrate_t<double>(n, k, seed, first, c, wscale, d_partials, nblocks, d_scratch, chunk, ev, ga, s);
+      return integrate_t<double>(n, k, seed, first, c, wscale, d_partials, nblocks, d_scratch, chunk, ev, ga,
+                                 d_gstage, s);
     return integrate_t<float>(n, k, seed, first, coup_cast<float>(c), wscale, d_partials, nblocks, d_scratch, chunk,
-                              ev, ga, s);
+                              ev, ga, d_gstage, s);
   }
   template <class T>
   static cudaError_t int_blocks_t(int* out, bool split) {
@@ -423,7 +464,7 @@ constexpr ProcVTable make_vtable(double flops_me, double flops_ps) {
   return ProcVTable{hg_process_info_t{P::n_ext, P::n_final, P::n_hel_total, P::n_hel_nonzero, P::n_diagrams,
                                       P::n_amplitudes, P::n_flows, P::n_draws, P::avg_factor, flops_me, flops_ps},
                     &Launch<P>::me, &Launch<P>::ps, &Launch<P>::integrate, &Launch<P>::int_blocks_per_sm,
-                    &Launch<P>::scratch_bytes, &Launch<P>::split_step, &Launch<P>::has_hadronic};
+                    &Launch<P>::scratch_bytes, &Launch<P>::split_step, &Launch<P>::has_hadronic, &Launch<P>::gstage};
 }
 
 }  // namespace hg

@@ -35,6 +35,24 @@ struct SmemStage {
   // (shared instruction-cache lines).  Every thread of the block must call me2().
   __device__ __forceinline__ void sync() const { __syncthreads(); }
 };
+// Staging area in GLOBAL memory (P::stage_global: W + 4 jets, 738 words = 5.9 KB per event in fp64, which in shared
+// memory leaves room for one pair of warps per SM).  Same layout [slot][event], event = the block's slot in a
+// buffer of gridDim.x * (events per block) columns, so a warp touches 32 consecutive words; the accesses go to
+// L2 (volatile: not cached in L1, not hoisted by the compiler).  The working set of a persistent grid -- 148 blocks
+// x 128 events x 5.9 KB = 112 MB -- fits the 126 MB L2.  What is bought is occupancy: the number of warps is then
+// limited by registers only.
+template <class T>
+struct GmemStage {
+  T* b;            // buffer + column of this event
+  int64_t stride;  // columns of the buffer
+  int half;
+  __device__ __forceinline__ int lo() const { return half; }
+  __device__ __forceinline__ int hi() const { return half + 1; }
+  __device__ __forceinline__ bool own(int h) const { return half == h; }
+  __device__ __forceinline__ T get(int s) const { return ((volatile T*)b)[s * stride]; }
+  __device__ __forceinline__ void put(int s, T v) const { ((volatile T*)b)[s * stride] = v; }
+  __device__ __forceinline__ void sync() const { __syncthreads(); }   // also orders the block's global accesses
+};
 #endif
 template <class T>
 struct HostStage {

@@ -448,11 +448,16 @@ class CodeGen(Emitter):
         if not p.mass:
             return 'T(0)'
         self.need_rm2.add(p.mass)
-        self._reg('rm2_%s' % p.mass, 'T', 0)
+        self._reg('rm2_%s' % p.mass, 'cx<T>', 0)
         return self._ref('rm2_%s' % p.mass)
 
-    @staticmethod
-    def _cpl(name):
+    # couplings that contain m_W or m_Z: complex in the paper's complex-mass option (Eq. 55)
+    COMPLEX_COUPLINGS = ('gtth', 'gwwh', 'gzzh', 'ghhh')
+
+    @classmethod
+    def _cpl(cls, name):
+        if name in cls.COMPLEX_COUPLINGS:
+            return 'mk<T>(c.%s, c.%s_i)' % (name, name)
         return 'c.%s' % name if name else 'T(0)'
 
     def _name(self, nd, vi, hel):
@@ -883,7 +888,13 @@ class CodeGen(Emitter):
                     terms.append('c.%s * c.%s' % (self.legs[l].particle.mass, self.legs[l].particle.mass))
             define('q2_%d' % m, 'T', ' + '.join(terms), cheap=True)
         for mass in sorted(self.need_rm2):
-            define('rm2_%s' % mass, 'T', 'hrcp(c.%s * c.%s)' % (mass, mass), cheap=True)
+            # 1 / m_V^2, or 1 / (m_V^2 - i m_V Gamma_V) in the complex-mass option (c.cms = 1)
+            width = {'mw': 'ww', 'mz': 'wz'}.get(mass)
+            if width:
+                define('rm2_%s' % mass, 'cx<T>', 'crcp(c.%s * c.%s, -(c.cms * c.%s * c.%s))' % (mass, mass, mass, width),
+                       cheap=True)
+            else:
+                define('rm2_%s' % mass, 'cx<T>', 'mk<T>(hrcp(c.%s * c.%s), T(0))' % (mass, mass), cheap=True)
         for (m, mass, width, spin), name in sorted(self.need_d.items()):
             sign = '' if spin == 'V' else '-'
             den = 'q2_%d' % m if not mass else '(q2_%d - c.%s * c.%s)' % (m, mass, mass)

@@ -84,6 +84,9 @@ KFROMP = set()
 # processes whose FFV closings do NOT go through dressed spinors (gen/emit.py DRESS): config 4 would need 174 staged
 # words instead of 142 and fall from 12 to 8 warps per SM
 NO_DRESS = {4}
+# staged processes whose staging area lives in GLOBAL memory (csrc/hg_stage.cuh GmemStage): W + 4 jets needs 738
+# words per event, one pair of warps per SM in shared memory
+STAGE_GLOBAL = {9}
 
 
 def build(spec, last=None):
@@ -206,6 +209,7 @@ struct P%(pid)d {
   static constexpr int n_diagrams = %(n_diagrams)d, n_amplitudes = %(n_amplitudes)d, n_flows = %(n_flows)d;
   static constexpr int n_draws = %(n_draws)d;
   static constexpr int n_stage = %(n_stage)d;  // words per event of the staging area (0: not staged)
+  static constexpr bool stage_global = %(stage_global)s;  // the staging area is global memory, not shared
   // hg_integrate_step as phase-space kernel + compaction + |M|^2 kernel per chunk (true) or one fused kernel
   static constexpr bool split_step = %(split_step)s;
   static constexpr double avg_factor = %(avg)s;
@@ -240,6 +244,7 @@ struct P%(pid)d {
            n_ext=row['n_ext'], n_final=row['n_final'], n_rambo=n_rambo, n_hel_total=row['n_hel_total'],
            n_hel_nonzero=row['n_hel_nonzero'], n_diagrams=row['n_diagrams'], n_amplitudes=row['n_amplitudes'],
            n_flows=row['n_flows'], n_draws=row['n_draws'], n_stage=cg.n_stage,
+           stage_global='true' if spec.pid in STAGE_GLOBAL else 'false',
            split_step='true' if (cg.n_stage > 0 or spec.pid in SPLIT_STEP) else 'false', avg=repr(row['avg_factor']),
            me_threads=ME_THREADS.get(spec.pid, 128), n_jets=len(jets), n_leps=len(leps), jets=arr(jets),
            leps=arr(leps), gen_call=gen_call, has_had='true' if had_call else 'false',

@@ -1,7 +1,8 @@
 // hostcheck.cpp -- test harness (tests/test_generated_host.py): evaluates the generated matrix elements in fp64 on the
 // HOST (the device library compiles as plain C++) for momenta read from stdin, so that the emitted code can be
 // checked without a GPU (tests/test_generated_host.py).  Never linked into libhg.so.
-//   input : lines "pid  E px py pz  E px py pz ..." (n_ext momenta, leg order of include/hg.h)
+//   input : lines "pid  E px py pz  E px py pz ..." (n_ext momenta, leg order of include/hg.h); a NEGATIVE pid
+//           evaluates process -pid with the complex-mass option (hg_params.complex_mass = 1)
 //   output: one line per input line, |Mbar|^2 with 17 significant digits
 #include <stdio.h>
 
@@ -36,10 +37,14 @@ bool eval(const Coup<double>& c) {
 int main() {
   hg_params par;
   default_params(&par);
-  const Coup<double> c = derive_couplings(par);
+  const Coup<double> c0 = derive_couplings(par);
+  par.complex_mass = 1;
+  const Coup<double> c1 = derive_couplings(par);
   int pid;
   while (scanf("%d", &pid) == 1) {
     bool ok = false;
+    const Coup<double>& c = pid < 0 ? c1 : c0;
+    if (pid < 0) pid = -pid;
     switch (pid) {
       case 1: ok = eval<P1>(c); break;
       case 2: ok = eval<P2>(c); break;

@@ -99,3 +99,59 @@ def test_cfg4_factorises_on_the_poles():
     # the directions matter event by event (spin correlations are there): the identity is not trivially true
     per_event = opr.me2(opr.config(4), fulls[:8], PAR) / (prod_me * 0.25 * decs[:8, 0] * decs[:8, 1] / (mt * gt) ** 4)
     assert np.abs(per_event - 1).max() > 0.05
+
+
+# ---------------------------------------------------------------------------------------- complex-mass option
+def test_complex_mass_is_the_analytic_continuation_in_the_masses():
+    """Eq. 55-56: replacing m_V^2 by m_V^2 - i m_V Gamma_V everywhere (propagator denominators,
+    q q / m_V^2 numerators, couplings) with mu_W^2 / mu_Z^2 = cos^2 theta_W is the same as evaluating the ZERO-WIDTH
+    formulas at the complex masses m_V sqrt(1 - i Gamma_Z / m_Z).  The oracle's explicit option branches
+    (complex_mass = 1) are compared with its plain formulas fed with complex mass parameters, for the processes whose
+    W and Z lines are all internal and end on conserved or non-conserved currents alike (Z* -> Z H H, W W / Z Z
+    fusion to H and H H).  A term that keeps the real mass (numerator, a coupling, the W width of Eq. 56) breaks the
+    equality at O(Gamma / m) = 3e-2 x its weight."""
+    from oracle import phase_space as ops
+    cms = dict(PAR, complex_mass=1)
+    fac = np.sqrt(complex(1.0, -PAR['gz'] / PAR['mz']))
+    cont = dict(PAR, mw=PAR['mw'] * fac, mz=PAR['mz'] * fac, gw=0.0, gz=0.0)
+    for cfg in (7, 10, 11):
+        p, _ = ops.generate(cfg, 4, 0, 6, opr.SQRT_S[cfg], PAR)
+        a = opr.me2(opr.config(cfg), p, cms)
+        b = opr.me2(opr.config(cfg), p, cont)
+        assert np.allclose(a, b, rtol=1e-12), (cfg, a, b)
+        plain = opr.me2(opr.config(cfg), p, PAR)
+        assert np.abs(a / plain - 1).max() > 1e-5          # the option does something
+    # Eq. 56 fixes the W width; in the narrow limit the option changes nothing
+    assert abs(sm.effective_widths(cms)[0] - PAR['mw'] * PAR['gz'] / PAR['mz']) < 1e-15
+    narrow = dict(PAR, gw=1e-12, gz=1e-12)
+    p, _ = ops.generate(11, 4, 0, 4, opr.SQRT_S[11], PAR)
+    assert np.allclose(opr.me2(opr.config(11), p, dict(narrow, complex_mass=1)), opr.me2(opr.config(11), p, narrow),
+                       rtol=1e-12)
+
+
+def test_complex_mass_ww_fusion_closed_form():
+    """The W W fusion closed form (tests/test_oracle_closed_forms.py) with the complex-mass option: the W W H coupling
+    becomes g_W mu_W, |mu_W|^2 = m_W^2 sqrt(1 + (Gamma_W/m_W)^2), and both space-like propagators carry Eq. 56's
+    width."""
+    from oracle import phase_space as ops
+    from oracle import philox
+    par = dict(PAR, mt=0.0, gt=0.0, complex_mass=1)
+    proc = opr.Process('ub_hdt', ['u', 'b'], ['h', 'd', 't'], ['udw', 'tbw', 'wwh'])
+    n, rs = 16, 1000.0
+    u = philox.uniforms(5, 0, n, 12, 3)
+    masses = np.stack([np.full(n, PAR['mh']), np.zeros(n), np.zeros(n)], 1)
+    k, _ = ops.rambo_massive(u, masses, rs)
+    p = np.zeros((n, 5, 4))
+    p[:, 0] = [rs / 2, 0, 0, rs / 2]
+    p[:, 1] = [rs / 2, 0, 0, -rs / 2]
+    p[:, 2:] = k
+    gw, mw = sm.couplings(par)['gw'], par['mw']
+    gam = par['mw'] * par['gz'] / par['mz']
+    q1 = p[:, 0] - p[:, 3]
+    q2 = p[:, 1] - p[:, 4]
+    d1 = (inputs.mdot(q1, q1) - mw * mw) ** 2 + (mw * gam) ** 2
+    d2 = (inputs.mdot(q2, q2) - mw * mw) ** 2 + (mw * gam) ** 2
+    mu2 = mw * mw * math.sqrt(1 + (gam / mw) ** 2)
+    want = (gw ** 2 / 2) ** 2 * gw ** 2 * mu2 * 16 * inputs.mdot(p[:, 0], p[:, 1]) * inputs.mdot(p[:, 3], p[:, 4]) \
+        / (d1 * d2) * 9 / 36
+    assert np.allclose(opr.me2(proc, p, par), want, rtol=1e-11)
