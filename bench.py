@@ -385,17 +385,20 @@ def run_gpu(args):
     pname = args.dtype
     el = 8 if prec == api.HG_F64 else 4
     p, _, _ = ctx.hg_gen_phase_space(cfg, prec, SEED, first, n, rs, want_pass=False)
-    hp = torch.empty(p.shape, dtype=p.dtype).pin_memory()
-    hp.copy_(p)
+    pf = p[2:].contiguous()                      # the events are in the partonic CM frame: ship the final-state legs
+    hp = torch.empty(pf.shape, dtype=p.dtype).pin_memory()
+    hp.copy_(pf)
     hme = torch.empty((n,), dtype=p.dtype).pin_memory()
-    del p
+    del p, pf
     for _ in range(3):
-        ctx.hg_matrix_element_host(cfg, prec, hp, hme)
-    e2e_ms = statistics.mean(_events_ms(torch, lambda: ctx.hg_matrix_element_host(cfg, prec, hp, hme), args.steps))
+        ctx.hg_matrix_element_host_cm(cfg, prec, rs, hp, hme)
+    e2e_ms = statistics.mean(_events_ms(torch, lambda: ctx.hg_matrix_element_host_cm(cfg, prec, rs, hp, hme),
+                                        args.steps))
     e2e = {'value': n / (e2e_ms * 1e-3), 'unit': UNIT, 'h2d_bytes_per_step': hp.numel() * el,
            'd2h_bytes_per_step': hme.numel() * el,
-           'what': 'hg_matrix_element_host: pinned host momenta -> H2D -> |Mbar|^2 kernel -> D2H per step, '
-                   'pipelined in 2^19-event chunks (copy of chunk i+1 overlaps the kernel of chunk i)'}
+           'what': 'hg_matrix_element_host_cm: pinned host momenta of the final-state legs (the incoming ones follow '
+                   'from sqrt(s_hat)) -> H2D -> |Mbar|^2 kernel -> D2H per step, pipelined in 2^19-event chunks (copy of '
+                   'chunk i+1 overlaps the kernel of chunk i)'}
     del hp, hme
 
     n_pass = acc[3] / world if world > 1 else acc[3]

@@ -167,6 +167,12 @@ int hg_matrix_element(hg_ctx* ctx, int process, int precision, int64_t n, const 
 int hg_matrix_element_host(hg_ctx* ctx, int process, int precision, int64_t n, const void* h_p,
                            void* h_me2, void* cuda_stream);
 
+/* The same for events given in the partonic centre-of-mass frame: the two incoming momenta are sqrt_s_hat/2 (1, 0, 0,
+ * +-1) and are NOT shipped; h_pfinal is [n_ext - 2][4][n] (final-state leg l of the process at row l - 2): 64 bytes
+ * per event less over PCIe, which is what bounds this call. */
+int hg_matrix_element_host_cm(hg_ctx* ctx, int process, int precision, int64_t n, double sqrt_s_hat,
+                              const void* h_pfinal, void* h_me2, void* cuda_stream);
+
 /* Steps a9-a10 on device arrays: w = pass * me2 * wps / (2 s_hat) * (hbar c)^2 [pb]; accumulates
  * acc = (sum w, sum w^2, n, n_pass) in double.  d_pass may be NULL (all pass).  Synchronises the stream;
  * acc is HOST memory, overwritten. */

@@ -16,7 +16,8 @@ HG_OK, HG_EINVAL, HG_ENOPROC, HG_ECUDA, HG_ENOTSET = 0, -1, -2, -3, -4
 
 # symbols include/hg.h declares (checked by tests/test_abi.py)
 SYMBOLS = ('hg_create', 'hg_destroy', 'hg_last_error', 'hg_default_params', 'hg_default_cuts', 'hg_process_info',
-           'hg_set_params', 'hg_gen_phase_space', 'hg_matrix_element', 'hg_matrix_element_host', 'hg_accumulate',
+           'hg_set_params', 'hg_gen_phase_space', 'hg_matrix_element', 'hg_matrix_element_host',
+           'hg_matrix_element_host_cm', 'hg_accumulate',
            'hg_integrate_step', 'hg_set_grid', 'hg_grid_refine', 'hg_default_hadronic', 'hg_set_hadronic')
 HG_GRID_MAX_BINS = 64
 # measurement helpers of include/hg_bench.h (bench.py only)
@@ -79,6 +80,7 @@ def load():
     L.hg_gen_phase_space.argtypes = [vp, i32, i32, u64, u64, i64, dbl, vp, vp, vp, vp]
     L.hg_matrix_element.argtypes = [vp, i32, i32, i64, vp, vp, vp]
     L.hg_matrix_element_host.argtypes = [vp, i32, i32, i64, vp, vp, vp]
+    L.hg_matrix_element_host_cm.argtypes = [vp, i32, i32, i64, dbl, vp, vp, vp]
     L.hg_accumulate.argtypes = [vp, i32, i64, vp, vp, vp, dbl, C.POINTER(dbl), vp]
     L.hg_integrate_step.argtypes = [vp, i32, i32, u64, u64, i64, dbl, C.POINTER(dbl), vp]
     L.hg_default_hadronic.argtypes = [i32, C.POINTER(hg_hadronic)]
@@ -229,6 +231,23 @@ class Context:
             raise ValueError('me2 must be a contiguous host %s tensor with %d elements' % (dt, n))
         self._check(self._L.hg_matrix_element_host(self._h, process, precision, n, _ptr(p), _ptr(me2),
                                                    _stream(stream)))
+        return me2
+
+    def hg_matrix_element_host_cm(self, process, precision, sqrt_s_hat, pfinal, me2=None, stream=None):
+        """pfinal: HOST tensor [n_ext - 2, 4, n] of the final-state momenta in the partonic centre-of-mass frame (the
+        incoming legs are sqrt_s_hat/2 (1, 0, 0, +-1) and are not shipped).  Returns a host tensor me2 [n]."""
+        n_fin = hg_process_info(process)['n_ext'] - 2
+        n = pfinal.numel() // (4 * n_fin)
+        dt = _dtype(precision)
+        if pfinal.device.type != 'cpu' or pfinal.dtype != dt or not pfinal.is_contiguous() or \
+                pfinal.numel() != 4 * n_fin * n:
+            raise ValueError('pfinal must be a contiguous host %s tensor [n_ext - 2, 4, n]' % dt)
+        if me2 is None:
+            me2 = torch.empty((n,), dtype=dt).pin_memory()
+        if me2.device.type != 'cpu' or me2.dtype != dt or not me2.is_contiguous() or me2.numel() != n:
+            raise ValueError('me2 must be a contiguous host %s tensor with %d elements' % (dt, n))
+        self._check(self._L.hg_matrix_element_host_cm(self._h, process, precision, n, sqrt_s_hat, _ptr(pfinal),
+                                                      _ptr(me2), _stream(stream)))
         return me2
 
     def hg_accumulate(self, precision, me2, wps, passed, sqrt_s_hat, stream=None):

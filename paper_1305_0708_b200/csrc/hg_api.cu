@@ -483,13 +483,14 @@ int hg_matrix_element(hg_ctx* ctx, int process, int precision, int64_t n, const 
   int gblocks = 0;
   cudaError_t e = ensure_gstage(ctx, vt, precision, &gblocks);
   if (e != cudaSuccess) return fail_cuda(ctx, e, "hg_matrix_element: global staging buffer");
-  e = vt->me(precision, n, d_p, d_me2, ctx->coup, ctx->d_gstage, gblocks, (cudaStream_t)cuda_stream);
+  e = vt->me(precision, n, d_p, d_me2, ctx->coup, ctx->d_gstage, gblocks, 0.0, (cudaStream_t)cuda_stream);
   if (e != cudaSuccess) return fail_cuda(ctx, e, "hg_matrix_element");
   return HG_OK;
 }
 
-int hg_matrix_element_host(hg_ctx* ctx, int process, int precision, int64_t n, const void* h_p, void* h_me2,
-                           void* cuda_stream) {
+// sqrt_s_hat > 0: h_p holds the final-state legs only (hg_matrix_element_host_cm)
+static int me_host(hg_ctx* ctx, int process, int precision, int64_t n, double sqrt_s_hat, const void* h_p,
+                   void* h_me2, void* cuda_stream) {
   int rc;
   const ProcVTable* vt = check(ctx, process, precision, n, &rc, "hg_matrix_element_host");
   if (!vt) return rc;
@@ -502,7 +503,7 @@ int hg_matrix_element_host(hg_ctx* ctx, int process, int precision, int64_t n, c
   // copy stream) overlaps the kernel and the D2H copy of chunk i (on the caller's stream).  The host array is
   // [n_ext][4][n], so one chunk is 4 n_ext strided rows: one cudaMemcpy2DAsync.
   const size_t el = precision == HG_F64 ? 8 : 4;
-  const int rows = 4 * vt->info.n_ext;
+  const int rows = 4 * (sqrt_s_hat > 0.0 ? vt->info.n_ext - 2 : vt->info.n_ext);
   const int64_t chunk = n < kHostChunk ? n : kHostChunk;
   const size_t in_bytes = el * rows * (size_t)chunk, out_bytes = el * (size_t)chunk;
   const size_t buf_bytes = (in_bytes + out_bytes + 255) / 256 * 256;
@@ -541,7 +542,8 @@ int hg_matrix_element_host(hg_ctx* ctx, int process, int precision, int64_t n, c
                             el * (size_t)m, rows, cudaMemcpyHostToDevice, ctx->copy_stream);
     if (e == cudaSuccess) e = cudaEventRecord(ctx->ev_h2d[b], ctx->copy_stream);
     if (e == cudaSuccess) e = cudaStreamWaitEvent(s, ctx->ev_h2d[b], 0);
-    if (e == cudaSuccess) e = vt->me(precision, m, d_in, d_out, ctx->coup, ctx->d_gstage, gblocks, s);
+    if (e == cudaSuccess)
+      e = vt->me(precision, m, d_in, d_out, ctx->coup, ctx->d_gstage, gblocks, 0.5 * sqrt_s_hat, s);
     if (e == cudaSuccess)
       e = cudaMemcpyAsync((char*)h_me2 + el * (size_t)off, d_out, el * (size_t)m, cudaMemcpyDeviceToHost, s);
     if (e == cudaSuccess) e = cudaEventRecord(ctx->ev_free[b], s);
@@ -549,6 +551,19 @@ int hg_matrix_element_host(hg_ctx* ctx, int process, int precision, int64_t n, c
   if (e == cudaSuccess) e = cudaStreamSynchronize(s);
   if (e != cudaSuccess) return fail_cuda(ctx, e, "hg_matrix_element_host");
   return HG_OK;
+}
+
+int hg_matrix_element_host(hg_ctx* ctx, int process, int precision, int64_t n, const void* h_p, void* h_me2,
+                           void* cuda_stream) {
+  return me_host(ctx, process, precision, n, 0.0, h_p, h_me2, cuda_stream);
+}
+
+int hg_matrix_element_host_cm(hg_ctx* ctx, int process, int precision, int64_t n, double sqrt_s_hat,
+                              const void* h_pfinal, void* h_me2, void* cuda_stream) {
+  if (!ctx) return HG_EINVAL;
+  if (!finite_pos(sqrt_s_hat))
+    return fail(ctx, HG_EINVAL, "hg_matrix_element_host_cm: sqrt_s_hat must be finite and > 0");
+  return me_host(ctx, process, precision, n, sqrt_s_hat, h_pfinal, h_me2, cuda_stream);
 }
 
 // finalize partials -> acc (host), synchronising the stream

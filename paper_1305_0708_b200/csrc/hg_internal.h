@@ -32,8 +32,9 @@ struct ProcVTable {
   hg_process_info_t info;
   // hg_matrix_element: p [n_ext][4][n] -> me2 [n]
   // d_gstage / gblocks: global staging buffer and grid of processes that stage in global memory (gstage below)
+  // ebeam > 0: d_p holds the final-state legs only, the incoming momenta are ebeam (1, 0, 0, +-1)
   cudaError_t (*me)(int prec, int64_t n, const void* d_p, void* d_me2, const Coup<double>& c, void* d_gstage,
-                    int gblocks, cudaStream_t s);
+                    int gblocks, double ebeam, cudaStream_t s);
   // hg_gen_phase_space
   cudaError_t (*ps)(int prec, int64_t n, const PsConst& k, uint64_t seed, uint64_t first, void* d_p,
                     void* d_wps, uint8_t* d_pass, cudaStream_t s);

@@ -174,6 +174,9 @@ template <int N>
 HG_HD double rambo_massive(const double* u, const double* m2, double msum, double rs, Mom<double>* k) {
   rambo_massless<N>(u, rs, k);
   double xi = sqrt(1.0 - (msum / rs) * (msum / rs));
+  // at most 12 Newton steps (the oracle always takes 12); quadratic convergence reaches the fixed point in 4-6, after
+  // which a step changes xi by at most an ulp: stop once the energy sum is met to 4 ulp
+#pragma unroll 1
   for (int it = 0; it < 12; ++it) {
     double f = -rs, df = 0;
 #pragma unroll
@@ -184,6 +187,7 @@ HG_HD double rambo_massive(const double* u, const double* m2, double msum, doubl
       df += xi * e2 / en;
     }
     xi -= f / df;
+    if (fabs(f) <= 8.9e-16 * rs) break;
   }
   double ksum = 0, prod = 1, den = 0;
 #pragma unroll

@@ -29,7 +29,7 @@ namespace hg {
 constexpr int kSmemPerSM = 227 * 1024;
 template <class P>
 constexpr int kSplit = P::n_stage > 0 ? 2 : 1;
-constexpr int kGlobalStageThreads = 256;   // global staging area: 4 pairs per block, limited by registers
+constexpr int kGlobalStageThreads = 256;   // global staging area: 4 pairs per block walk the code together
 template <class P, class T>
 constexpr int stage_threads(int want) {
   if (P::n_stage == 0) return want;
@@ -58,7 +58,7 @@ __device__ __forceinline__ bool ev_owner() {
 
 // me2 of one event.  Staged: the staging area of the event is shared memory laid out [slot][event] (hg_stage.cuh);
 // every thread of the block must call; the total is returned to the owner thread of the pair.
-// gstage: global staging buffer of gridDim.x * EPB columns (P::stage_global), else unused.
+// gstage: global staging buffer, one region of n_stage x EPB words per block (P::stage_global), else unused.
 template <class P, class T, int THREADS>
 __device__ __forceinline__ T me2_event(const Mom<T>* q, const Coup<T>& c, T* gstage) {
   if constexpr (P::n_stage > 0) {
@@ -69,7 +69,7 @@ __device__ __forceinline__ T me2_event(const Mom<T>* q, const Coup<T>& c, T* gst
     const int half = (threadIdx.x >> 5) & 1;
     T r;
     if constexpr (P::stage_global) {
-      const GmemStage<T> st{gstage + (int64_t)blockIdx.x * EPB + ev, (int64_t)gridDim.x * EPB, half};
+      const GmemStage<T, EPB> st{gstage + (int64_t)blockIdx.x * (P::n_stage * EPB) + ev, half};
       r = P::template me2<T>(q, c, st);
     } else {
       const SmemStage<T, EPB> st{reinterpret_cast<T*>(hg_stage_smem) + ev, half};
@@ -88,16 +88,23 @@ __device__ __forceinline__ T me2_event(const Mom<T>* q, const Coup<T>& c, T* gst
 // Grid: one block per EPB events, or (P::stage_global) a persistent grid that strides over the batches, each block
 // keeping its EPB columns of the global staging buffer.
 template <class P, class T, int THREADS>
+// ebeam > 0: p holds the FINAL-STATE legs only (leg l at row l - 2) and the incoming momenta are ebeam (1, 0, 0, +-1)
+// (hg_matrix_element_host_cm: 64 bytes per event less over PCIe); ebeam <= 0: all n_ext legs.
 __global__ void __launch_bounds__(THREADS) me_kernel(const T* __restrict__ p, T* __restrict__ me2, int64_t n,
-                                                     const Coup<T> c, T* gstage) {
+                                                     const Coup<T> c, T* gstage, T ebeam) {
   constexpr int EPB = THREADS / kSplit<P>;
+  const int l0 = ebeam > T(0) ? 2 : 0;     // grid-uniform
   for (int64_t base = (int64_t)blockIdx.x * EPB; base < n; base += (int64_t)gridDim.x * EPB) {   // block-uniform
     const int64_t e0 = base + ev_local<P>();
     const int64_t e = e0 < n ? e0 : n - 1;  // no early exit: a staged me2 holds block-wide rendezvous
     Mom<T> q[P::n_ext];
+    q[0] = mkmom<T>(ebeam, T(0), T(0), ebeam);
+    q[1] = mkmom<T>(ebeam, T(0), T(0), -ebeam);
 #pragma unroll
     for (int l = 0; l < P::n_ext; ++l)
-      q[l] = mkmom<T>(p[(l * 4 + 0) * n + e], p[(l * 4 + 1) * n + e], p[(l * 4 + 2) * n + e], p[(l * 4 + 3) * n + e]);
+      if (l >= l0)
+        q[l] = mkmom<T>(p[((l - l0) * 4 + 0) * n + e], p[((l - l0) * 4 + 1) * n + e], p[((l - l0) * 4 + 2) * n + e],
+                        p[((l - l0) * 4 + 3) * n + e]);
     const T r = me2_event<P, T, THREADS>(q, c, gstage);
     if (e0 < n && ev_owner<P>()) me2[e0] = r;
   }
@@ -301,7 +308,7 @@ struct Launch {
   // gblocks: blocks of the persistent grid, d_gstage: global staging buffer (P::stage_global only, gstage())
   template <class T>
   static cudaError_t me_t(int64_t n, const void* d_p, void* d_me2, const Coup<T>& c, void* d_gstage, int gblocks,
-                          cudaStream_t s) {
+                          double ebeam, cudaStream_t s) {
     constexpr int TH = me_thr<T>();
     constexpr size_t smem = stage_bytes<P, T, TH>();
     cudaError_t err = allow_smem(me_kernel<P, T, TH>, smem);
@@ -309,13 +316,13 @@ struct Launch {
     constexpr int EPB = TH / kSplit<P>;
     unsigned grid = (unsigned)((n + EPB - 1) / EPB);
     if (P::stage_global && grid > (unsigned)gblocks) grid = (unsigned)gblocks;
-    me_kernel<P, T, TH><<<grid, TH, smem, s>>>((const T*)d_p, (T*)d_me2, n, c, (T*)d_gstage);
+    me_kernel<P, T, TH><<<grid, TH, smem, s>>>((const T*)d_p, (T*)d_me2, n, c, (T*)d_gstage, T(ebeam));
     return cudaGetLastError();
   }
   static cudaError_t me(int prec, int64_t n, const void* d_p, void* d_me2, const Coup<double>& c, void* d_gstage,
-                        int gblocks, cudaStream_t s) {
-    if (prec == HG_F64) return me_t<double>(n, d_p, d_me2, c, d_gstage, gblocks, s);
-    return me_t<float>(n, d_p, d_me2, coup_cast<float>(c), d_gstage, gblocks, s);
+                        int gblocks, double ebeam, cudaStream_t s) {
+    if (prec == HG_F64) return me_t<double>(n, d_p, d_me2, c, d_gstage, gblocks, ebeam, s);
+    return me_t<float>(n, d_p, d_me2, coup_cast<float>(c), d_gstage, gblocks, ebeam, s);
   }
   // Global staging buffer: resident blocks per SM of the two kernels that evaluate me2 (the smaller one) and the
   // bytes of a buffer for n_sm * that many blocks; 0 blocks / 0 bytes for processes that stage in shared memory.

@@ -36,21 +36,21 @@ struct SmemStage {
   __device__ __forceinline__ void sync() const { __syncthreads(); }
 };
 // Staging area in GLOBAL memory (P::stage_global: W + 4 jets, 738 words = 5.9 KB per event in fp64, which in shared
-// memory leaves room for one pair of warps per SM).  Same layout [slot][event], event = the block's slot in a
-// buffer of gridDim.x * (events per block) columns, so a warp touches 32 consecutive words; the accesses go to
-// L2 (volatile: not cached in L1, not hoisted by the compiler).  The working set of a persistent grid -- 148 blocks
-// x 128 events x 5.9 KB = 112 MB -- fits the 126 MB L2.  What is bought is occupancy: the number of warps is then
-// limited by registers only.
-template <class T>
+// memory leaves room for one pair of warps per SM).  Every block of the persistent grid owns a region laid out
+// [slot][event of the block] like the shared-memory area, so a warp touches 32 consecutive words and slot s sits at
+// the COMPILE-TIME offset s * STRIDE from one base pointer (with a run-time stride ptxas hoisted the 738 slot
+// addresses out of the loops and spilled them: 13 KB of stack).  The accesses go to L2 (volatile: not cached in L1,
+// not hoisted by the compiler); the working set of the grid, 592 blocks x 32 events x 5.9 KB = 112 MB, fits the
+// 126 MB L2.  What is bought is occupancy: the number of warps is then limited by registers only.
+template <class T, int STRIDE>
 struct GmemStage {
-  T* b;            // buffer + column of this event
-  int64_t stride;  // columns of the buffer
+  T* b;            // region of the block + event in the block
   int half;
   __device__ __forceinline__ int lo() const { return half; }
   __device__ __forceinline__ int hi() const { return half + 1; }
   __device__ __forceinline__ bool own(int h) const { return half == h; }
-  __device__ __forceinline__ T get(int s) const { return ((volatile T*)b)[s * stride]; }
-  __device__ __forceinline__ void put(int s, T v) const { ((volatile T*)b)[s * stride] = v; }
+  __device__ __forceinline__ T get(int s) const { return ((volatile T*)b)[s * STRIDE]; }
+  __device__ __forceinline__ void put(int s, T v) const { ((volatile T*)b)[s * STRIDE] = v; }
   __device__ __forceinline__ void sync() const { __syncthreads(); }   // also orders the block's global accesses
 };
 #endif
@@ -164,6 +164,21 @@ HG_HD Vc<T> ld_pol(const St& st, int s, int flip) {
     v.c[3].re = -v.c[3].re;
   }
   return v;
+}
+
+// the same in the light-cone form the FFV vertices use (hg_helas.cuh Pol<T>; declared there, defined via the staged
+// five words): flip != 0 gives the helicity -1 vector
+template <class T>
+struct Pol;
+template <class T, class St>
+HG_HD Pol<T> ld_pol_lc(const St& st, int s, int flip) {
+  const T sg = flip ? T(-1) : T(1);
+  const T v1r = sg * st.get(s), v1i = st.get(s + 1), v2r = sg * st.get(s + 2), v2i = st.get(s + 3);
+  Pol<T> p;
+  p.v3 = sg * st.get(s + 4);
+  p.ur = mk<T>(v1r + v2i, v1i - v2r);
+  p.ll = mk<T>(v1r - v2i, v1i + v2r);
+  return p;
 }
 
 }  // namespace hg

@@ -84,9 +84,11 @@ KFROMP = set()
 # processes whose FFV closings do NOT go through dressed spinors (gen/emit.py DRESS): config 4 would need 174 staged
 # words instead of 142 and fall from 12 to 8 warps per SM
 NO_DRESS = {4}
-# staged processes whose staging area lives in GLOBAL memory (csrc/hg_stage.cuh GmemStage): W + 4 jets needs 738
-# words per event, one pair of warps per SM in shared memory
-STAGE_GLOBAL = {9}
+# staged processes whose staging area lives in GLOBAL memory (csrc/hg_stage.cuh GmemStage).  Measured for W + 4 jets
+# (738 words per event: one pair of warps per SM in shared memory): 8 warps per SM through L2 are SLOWER than 2 warps
+# through shared memory, 34.9 ms against 26.5 ms per 2^18 events in fp64, 27.2 against 12.9 ms in fp32, whether the
+# 8 warps sit in one block or four (profiles/r02_notes.md): the option stays off.
+STAGE_GLOBAL = set()
 
 
 def build(spec, last=None):

@@ -191,6 +191,10 @@ def test_matrix_element_host_pipeline_multichunk(ctx, api, cfg, prec):
         got = ctx.hg_matrix_element_host(cfg, pr, hp, out[:n])
         assert torch.equal(got, ref.cpu())
         assert bool((out[n:] == -7.0).all())
+    # final-state legs only (hg_matrix_element_host_cm, the e2e leg of bench.py): same bits
+    hf = torch.empty(p[2:].shape, dtype=p.dtype).pin_memory()
+    hf.copy_(p[2:])
+    assert torch.equal(ctx.hg_matrix_element_host_cm(cfg, pr, opr.SQRT_S[cfg], hf), ref.cpu())
     # not pinned, and a size just past one chunk
     m = (1 << 19) + 1
     hq = p[:, :, :m].contiguous().cpu()
