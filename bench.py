@@ -94,6 +94,15 @@ class ClockSampler:
         for line in self.proc.stdout:
             self.rows.append((time.time(), line.strip()))
 
+    def wait_first(self, timeout=5.0):
+        """Block until nvidia-smi has delivered its first sample (its start-up can exceed a short timed region)."""
+        t0 = time.time()
+        while self.proc is not None and not self.rows and time.time() - t0 < timeout:
+            time.sleep(0.02)
+
+    def n_between(self, t0, t1):
+        return sum(1 for t, _ in self.rows if t0 <= t <= t1)
+
     def stop(self, t0, t1):
         if self.proc is None:
             return {'sm_mhz': None, 'sm_max_mhz': None, 'reasons': ['nvidia-smi unavailable']}
@@ -101,7 +110,7 @@ class ClockSampler:
         self.proc.terminate()
         sm, smax, reasons = [], None, set()
         names = ('hw_slowdown', 'hw_thermal_slowdown', 'sw_thermal_slowdown', 'sw_power_cap')
-        rows = [r for t, r in self.rows if t0 <= t <= t1] or [r for _, r in self.rows]
+        rows = [r for t, r in self.rows if t0 <= t <= t1]
         for r in rows:
             f = [x.strip() for x in r.split(',')]
             try:
@@ -344,7 +353,7 @@ def run_gpu(args):
         acc = step()
     sampler = ClockSampler(local)
     sampler.start()
-    time.sleep(0.3)
+    sampler.wait_first()
     sync()
     t0 = time.time()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -367,7 +376,16 @@ def run_gpu(args):
     t1 = time.time()
     total_ms = e0.elapsed_time(e1)
     kern_ms = statistics.mean(a.elapsed_time(b) for a, b in per_step)
-    clocks = sampler.stop(t0, t1)
+    # K steps of a few ms can be shorter than a handful of 20 ms samples: keep the same load running (untimed) until the
+    # sampler has seen at least 5 samples under it, and say how many fell inside the timed region itself
+    in_region = sampler.n_between(t0, t1)
+    t_load = t1
+    while sampler.proc is not None and sampler.n_between(t0, t_load) < 5 and time.time() - t1 < 3.0:
+        step()
+        torch.cuda.synchronize()
+        t_load = time.time()
+    clocks = sampler.stop(t0, t_load)
+    clocks['samples_in_timed_region'] = in_region
     if world > 1:
         t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
