@@ -219,9 +219,9 @@ int hg_set_hadronic(hg_ctx* ctx, const hg_hadronic* h);
  * 0 = g[d][0] < ... < g[d][n_bins] = 1; the draw picks a bin uniformly and a point inside it, the event weight carries
  * the Jacobian prod_d n_bins (g[d][i+1] - g[d][i]).
  *
- * hg_set_grid: until reset, hg_gen_phase_space and hg_integrate_step of THE PROCESS THE GRID WAS MADE FOR sample
- * through d_grid ([n_draws][n_bins + 1] doubles, DEVICE memory owned by the caller, read at every call; 2 <= n_bins <=
- * HG_GRID_MAX_BINS).  If d_hist is not NULL ([n_draws][n_bins] doubles, device, caller-owned, caller-zeroed) every
+ * hg_set_grid: until reset, hg_gen_phase_space and hg_integrate_step sample through d_grid ([n_dim][n_bins + 1]
+ * doubles, DEVICE memory owned by the caller, read at every call; 2 <= n_bins <= HG_GRID_MAX_BINS).  n_dim must equal
+ * n_draws of the process of those calls, else they return HG_EINVAL (a grid belongs to one process).  If d_hist is not NULL ([n_draws][n_bins] doubles, device, caller-owned, caller-zeroed) every
  * hg_integrate_step ADDS the sum of w^2 of the passing events per (draw, bin) to it: the grid-optimisation step.
  * Summation order is fixed (no atomics): same inputs, same histogram.  d_grid == NULL returns to flat sampling.
  *
@@ -229,7 +229,7 @@ int hg_set_hadronic(hg_ctx* ctx, const hg_hadronic* h);
  * accumulated histogram -- smoothing over neighbouring bins, compression ((1 - s)/ln(1/s))^alpha, re-binning to equal
  * content; a variable whose histogram is empty or not finite keeps its edges.  h_grid is updated in place. */
 #define HG_GRID_MAX_BINS 64
-int hg_set_grid(hg_ctx* ctx, const double* d_grid, int n_bins, double* d_hist);
+int hg_set_grid(hg_ctx* ctx, const double* d_grid, int n_dim, int n_bins, double* d_hist);
 int hg_grid_refine(int n_dim, int n_bins, const double* h_hist, double alpha, double* h_grid);
 
 #ifdef __cplusplus

@@ -85,7 +85,7 @@ def load():
     L.hg_integrate_step.argtypes = [vp, i32, i32, u64, u64, i64, dbl, C.POINTER(dbl), vp]
     L.hg_default_hadronic.argtypes = [i32, C.POINTER(hg_hadronic)]
     L.hg_set_hadronic.argtypes = [vp, C.POINTER(hg_hadronic)]
-    L.hg_set_grid.argtypes = [vp, vp, i32, vp]
+    L.hg_set_grid.argtypes = [vp, vp, i32, i32, vp]
     L.hg_grid_refine.argtypes = [i32, i32, vp, dbl, vp]
     L.hg_measure_fma_peak.argtypes = [vp, i32, C.POINTER(dbl), vp]
     L.hg_set_profiling.argtypes = [vp, i32]
@@ -277,14 +277,14 @@ class Context:
         sampling; hist: CUDA float64 tensor [n_draws, n_bins] that hg_integrate_step adds sum w^2 per bin to."""
         if grid is None:
             self._grid = self._hist = None
-            self._check(self._L.hg_set_grid(self._h, None, 0, None))
+            self._check(self._L.hg_set_grid(self._h, None, 0, 0, None))
             return
         n_dim, nb1 = grid.shape
         self._check_tensor(grid, HG_F64, n_dim * nb1, 'grid', torch.float64)
         if hist is not None:
             self._check_tensor(hist, HG_F64, n_dim * (nb1 - 1), 'hist', torch.float64)
         self._grid, self._hist = grid, hist
-        self._check(self._L.hg_set_grid(self._h, _ptr(grid), nb1 - 1, _ptr(hist)))
+        self._check(self._L.hg_set_grid(self._h, _ptr(grid), n_dim, nb1 - 1, _ptr(hist)))
 
     def hg_set_profiling(self, on):
         self._check(self._L.hg_set_profiling(self._h, 1 if on else 0))

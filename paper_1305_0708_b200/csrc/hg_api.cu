@@ -52,8 +52,9 @@ struct hg_ctx {
   size_t scratch_bytes = 0;
   bool hadronic = false;           // hg_set_hadronic
   hg_hadronic had;
-  const double* d_grid = nullptr;  // hg_set_grid: caller-owned [n_draws][grid_nb + 1]
+  const double* d_grid = nullptr;  // hg_set_grid: caller-owned [grid_ndim][grid_nb + 1]
   int grid_nb = 0;
+  int grid_ndim = 0;
   double* d_hist = nullptr;        // caller-owned [n_draws][grid_nb], or NULL
   void* d_gstage = nullptr;          // global staging buffer of processes that stage in global memory (W + 4 jets)
   size_t gstage_bytes = 0;
@@ -456,6 +457,8 @@ int hg_gen_phase_space(hg_ctx* ctx, int process, int precision, uint64_t seed, u
   const ProcVTable* vt = check(ctx, process, precision, n, &rc, "hg_gen_phase_space");
   if (!vt) return rc;
   if ((rc = check_rs(ctx, vt, process, sqrt_s_hat, "hg_gen_phase_space")) != HG_OK) return rc;
+  if (ctx->d_grid && ctx->grid_ndim != vt->info.n_draws)
+    return fail(ctx, HG_EINVAL, "hg_gen_phase_space: the grid set by hg_set_grid has another number of draws than this process");
   if (n == 0) return HG_OK;
   if (!d_p || !d_wps) return fail(ctx, HG_EINVAL, "hg_gen_phase_space: d_p / d_wps is NULL");
   if (misaligned(d_p, precision == HG_F64 ? 8 : 4) || misaligned(d_wps, precision == HG_F64 ? 8 : 4))
@@ -617,6 +620,8 @@ int hg_integrate_step(hg_ctx* ctx, int process, int precision, uint64_t seed, ui
   if (!vt) return rc;
   if (!acc) return fail(ctx, HG_EINVAL, "hg_integrate_step: acc is NULL");
   if ((rc = check_rs(ctx, vt, process, sqrt_s_hat, "hg_integrate_step")) != HG_OK) return rc;
+  if (ctx->d_grid && ctx->grid_ndim != vt->info.n_draws)
+    return fail(ctx, HG_EINVAL, "hg_integrate_step: the grid set by hg_set_grid has another number of draws than this process");
   acc[0] = acc[1] = acc[2] = acc[3] = 0.0;
   if (n == 0) return HG_OK;
   HG_ON_DEVICE(ctx, "hg_integrate_step");
@@ -719,18 +724,20 @@ int hg_set_hadronic(hg_ctx* ctx, const hg_hadronic* h) {
   return HG_OK;
 }
 
-int hg_set_grid(hg_ctx* ctx, const double* d_grid, int n_bins, double* d_hist) {
+int hg_set_grid(hg_ctx* ctx, const double* d_grid, int n_dim, int n_bins, double* d_hist) {
   if (!ctx) return HG_EINVAL;
   if (!d_grid) {
     ctx->d_grid = nullptr;
-    ctx->grid_nb = 0;
+    ctx->grid_nb = ctx->grid_ndim = 0;
     ctx->d_hist = nullptr;
     return HG_OK;
   }
   if (n_bins < 2 || n_bins > HG_GRID_MAX_BINS) return fail(ctx, HG_EINVAL, "hg_set_grid: n_bins out of range");
+  if (n_dim < 1 || n_dim > kHistMaxDim) return fail(ctx, HG_EINVAL, "hg_set_grid: n_dim out of range");
   if (misaligned(d_grid, 8) || misaligned(d_hist, 8)) return fail(ctx, HG_EINVAL, "hg_set_grid: misaligned pointer");
   ctx->d_grid = d_grid;
   ctx->grid_nb = n_bins;
+  ctx->grid_ndim = n_dim;
   ctx->d_hist = d_hist;
   return HG_OK;
 }

@@ -94,7 +94,9 @@ __global__ void __launch_bounds__(THREADS) me_kernel(const T* __restrict__ p, T*
                                                      const Coup<T> c, T* gstage, T ebeam) {
   constexpr int EPB = THREADS / kSplit<P>;
   const int l0 = ebeam > T(0) ? 2 : 0;     // grid-uniform
-  for (int64_t base = (int64_t)blockIdx.x * EPB; base < n; base += (int64_t)gridDim.x * EPB) {   // block-uniform
+  // one batch per block; only a persistent grid (global staging) strides over several
+  const int64_t stride = P::stage_global ? (int64_t)gridDim.x * EPB : n;
+  for (int64_t base = (int64_t)blockIdx.x * EPB; base < n; base += stride) {   // block-uniform
     const int64_t e0 = base + ev_local<P>();
     const int64_t e = e0 < n ? e0 : n - 1;  // no early exit: a staged me2 holds block-wide rendezvous
     Mom<T> q[P::n_ext];

@@ -697,3 +697,32 @@ def test_complex_mass_option(ctx, api, cfg):
     with pytest.raises(api.HgError):
         ctx.hg_set_params(bad)
     ctx.hg_set_params(api.hg_default_params())
+
+
+def test_sampling_mode_errors(ctx, api):
+    """Argument checks of the sampling modes: a grid belongs to one process; bin counts; hadronic parameters; the CM
+    variant of the host call needs sqrt_s_hat."""
+    from paper_1305_0708_b200.api import HgError
+    grid = torch.linspace(0, 1, 51, dtype=torch.float64, device='cuda').repeat(20, 1).contiguous()
+    try:
+        ctx.hg_set_grid(grid)                                   # 20 draws: W + 3 jets
+        ctx.hg_integrate_step(5, api.HG_F64, 1, 0, 100, 2000.0)
+        for call in (lambda: ctx.hg_integrate_step(3, api.HG_F64, 1, 0, 100, 1000.0),        # 16 draws
+                     lambda: ctx.hg_gen_phase_space(4, api.HG_F64, 1, 0, 100, 1500.0)):       # 24 draws
+            with pytest.raises(HgError) as ei:
+                call()
+            assert ei.value.code == api.HG_EINVAL
+    finally:
+        ctx.hg_set_grid(None)
+    big = torch.linspace(0, 1, 130, dtype=torch.float64, device='cuda').repeat(20, 1).contiguous()
+    with pytest.raises(HgError):
+        ctx.hg_set_grid(big)                                    # more than HG_GRID_MAX_BINS bins
+    h = api.hg_default_hadronic(5)
+    h.y_res_max = -1.0
+    with pytest.raises(HgError):
+        ctx.hg_set_hadronic(h)
+    ctx.hg_set_hadronic(None)
+    hp = torch.zeros((5, 4, 16), dtype=torch.float64)
+    with pytest.raises(HgError):
+        ctx.hg_matrix_element_host_cm(5, api.HG_F64, -1.0, hp)
+    assert ctx.hg_integrate_step(5, api.HG_F64, 1, 0, 100, 2000.0)[2] == 100     # the context is still usable
