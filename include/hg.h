@@ -127,7 +127,7 @@ int hg_create(hg_ctx** out, int cuda_device);
 void hg_destroy(hg_ctx* ctx);
 
 /* Text of the last error on this context (ctx-owned, valid until the next failing call).  ctx == NULL
- * returns the text of the last hg_create failure. */
+ * returns the text of the last failure of a call that has no context (hg_create, hg_accumulate_noalloc). */
 const char* hg_last_error(const hg_ctx* ctx);
 
 /* Default inputs of BASELINE.json (MZ=91.1876, MW=80.419, GZ=2.441, GW=2.048, 1/alpha=132.507,
@@ -178,6 +178,26 @@ int hg_matrix_element_host_cm(hg_ctx* ctx, int process, int precision, int64_t n
  * acc is HOST memory, overwritten. */
 int hg_accumulate(hg_ctx* ctx, int precision, int64_t n, const void* d_me2, const void* d_wps,
                   const uint8_t* d_pass, double sqrt_s_hat, double acc[4], void* cuda_stream);
+
+/* hg_accumulate for callers that cannot allocate (CUDA graph capture, tight serving loops, harnesses that forbid
+ * cudaMalloc): the same steps a9-a10 (section 4: w = |Mbar|^2 x phase-space weight x (hbar c)^2 / (2 s_hat),
+ * sums of w and w^2) with NO context and NO allocation -- the per-block partial sums go to a file-scope
+ * static __device__ array of the library (3 x 4096 doubles = 96 KB, held by every GPU that loads the library
+ * until the process exits) and the result is written to DEVICE memory the caller passes.
+ *   d_me2, d_wps [n] in (T), d_pass [n] in or NULL (all pass): device memory on the CURRENT device
+ *   d_acc [4] out, DEVICE memory (doubles, 8-byte aligned): (sum w, sum w^2, n, n_pass), overwritten
+ *   n <= HG_NOALLOC_MAX_EVENTS, else HG_EINVAL ("n exceeds HG_NOALLOC_MAX_EVENTS")
+ * Asynchronous on cuda_stream (two kernel launches, no synchronisation, no copy): d_acc is valid once the stream
+ * reaches that point.  Calls no cudaMalloc / cudaFree / allocating routine; the first call on a device looks up
+ * the address of the array (cudaGetSymbolAddress), later calls reuse it.  Block b sums the events
+ * [4096 b, 4096 (b + 1)) and the blocks are added in a fixed order: the result does not depend on the GPU.
+ * Every call SHARES the one array, which keeps the partial sums of the last call: each call overwrites the entries
+ * it reads (nothing needs clearing), but two calls that overlap on the GPU (different streams, or graphs replayed
+ * concurrently) race on it -- keep calls on one device in stream order.  There is no context to hold an error
+ * message: hg_last_error(NULL) returns the text of the last failure of this call. */
+#define HG_NOALLOC_MAX_EVENTS 16777216 /* 2^24 */
+int hg_accumulate_noalloc(int precision, int64_t n, const void* d_me2, const void* d_wps, const uint8_t* d_pass,
+                          double sqrt_s_hat, double* d_acc, void* cuda_stream);
 
 /* Steps a1-a10 in one call.
  * Configs 1, 3 and process 6: fused in one kernel -- each thread draws its event, builds momenta, applies the

@@ -17,7 +17,7 @@ HG_OK, HG_EINVAL, HG_ENOPROC, HG_ECUDA, HG_ENOTSET = 0, -1, -2, -3, -4
 # symbols include/hg.h declares (checked by tests/test_abi.py)
 SYMBOLS = ('hg_create', 'hg_destroy', 'hg_last_error', 'hg_default_params', 'hg_default_cuts', 'hg_process_info',
            'hg_set_params', 'hg_gen_phase_space', 'hg_matrix_element', 'hg_matrix_element_host',
-           'hg_matrix_element_host_cm', 'hg_accumulate',
+           'hg_matrix_element_host_cm', 'hg_accumulate', 'hg_accumulate_noalloc',
            'hg_integrate_step', 'hg_set_grid', 'hg_grid_refine', 'hg_default_hadronic', 'hg_set_hadronic')
 HG_GRID_MAX_BINS = 64
 # measurement helpers of include/hg_bench.h (bench.py only)
@@ -82,6 +82,7 @@ def load():
     L.hg_matrix_element_host.argtypes = [vp, i32, i32, i64, vp, vp, vp]
     L.hg_matrix_element_host_cm.argtypes = [vp, i32, i32, i64, dbl, vp, vp, vp]
     L.hg_accumulate.argtypes = [vp, i32, i64, vp, vp, vp, dbl, C.POINTER(dbl), vp]
+    L.hg_accumulate_noalloc.argtypes = [i32, i64, vp, vp, vp, dbl, vp, vp]
     L.hg_integrate_step.argtypes = [vp, i32, i32, u64, u64, i64, dbl, C.POINTER(dbl), vp]
     L.hg_default_hadronic.argtypes = [i32, C.POINTER(hg_hadronic)]
     L.hg_set_hadronic.argtypes = [vp, C.POINTER(hg_hadronic)]
@@ -138,6 +139,30 @@ def hg_grid_refine(hist, alpha, grid):
 
 def _dtype(precision):
     return torch.float64 if precision == HG_F64 else torch.float32
+
+
+HG_NOALLOC_MAX_EVENTS = 1 << 24
+
+
+def hg_accumulate_noalloc(precision, me2, wps, passed, sqrt_s_hat, acc, stream=None):
+    """hg_accumulate without a context and without any allocation (include/hg.h): acc is a CUDA float64 tensor of 4
+    elements that the CALLER provides; it receives (sum w, sum w^2, n, n_pass) asynchronously on the stream.  The
+    tensors must live on the current CUDA device."""
+    n = me2.numel()
+    dt = _dtype(precision)
+    for t, name, want in ((me2, 'me2', dt), (wps, 'wps', dt), (passed, 'pass', torch.uint8)):
+        if t is None and name == 'pass':
+            continue
+        if t.device.type != 'cuda' or t.dtype != want or not t.is_contiguous() or t.numel() != n:
+            raise ValueError('%s must be a contiguous CUDA %s tensor with %d elements' % (name, want, n))
+    if acc.device.type != 'cuda' or acc.dtype != torch.float64 or not acc.is_contiguous() or acc.numel() != 4:
+        raise ValueError('acc must be a contiguous CUDA float64 tensor with 4 elements')
+    L = load()
+    rc = L.hg_accumulate_noalloc(precision, n, _ptr(me2), _ptr(wps), _ptr(passed), float(sqrt_s_hat), _ptr(acc),
+                                 _stream(stream))
+    if rc != 0:
+        raise HgError(rc, L.hg_last_error(None).decode())
+    return acc
 
 
 def _stream(stream):

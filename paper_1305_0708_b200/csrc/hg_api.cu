@@ -4,6 +4,7 @@
 #include <stdio.h>
 #include <string.h>
 
+#include <mutex>
 #include <string>
 #include <vector>
 
@@ -80,6 +81,17 @@ static int fail_cuda(hg_ctx* ctx, cudaError_t e, const char* where) {
   return HG_ECUDA;
 }
 
+// failures of calls that have no context: the text goes where hg_last_error(NULL) reads it
+static int fail_noctx(int code, const char* msg) {
+  g_create_error = msg;
+  return code;
+}
+static int fail_cuda_noctx(cudaError_t e, const char* where) {
+  g_create_error = std::string(where) + ": " + cudaGetErrorString(e);
+  return HG_ECUDA;
+}
+constexpr int kNoAllocMaxDevices = 64;
+
 // Sums nb x 3 partials in a fixed order (deterministic result for a given grid).
 __global__ void finalize_kernel(const double* __restrict__ partials, int nb, double* __restrict__ acc) {
   __shared__ double sh[3][256];
@@ -148,6 +160,88 @@ __global__ void __launch_bounds__(256) accumulate_kernel(const T* __restrict__ m
     partials[3 * blockIdx.x] = a;
     partials[3 * blockIdx.x + 1] = b;
     partials[3 * blockIdx.x + 2] = c;
+  }
+}
+
+// ---- hg_accumulate_noalloc: steps a9-a10 with the partial sums in a file-scope device array (no allocation) ----
+constexpr int kNoAllocRange = 4096;                                   // events per block (16 per thread)
+constexpr int kNoAllocMaxBlocks = HG_NOALLOC_MAX_EVENTS / kNoAllocRange;   // 4096 blocks
+// The scratch of hg_accumulate_noalloc: [kNoAllocMaxBlocks][3] partial sums, 96 KB per GPU that loads the library.
+// In HOST code this name is a host-side stand-in, not a device address: the host passes the address it gets from
+// cudaGetSymbolAddress (noalloc_scratch below), once per device.
+static __device__ __align__(256) double hg_noalloc_partials[3 * kNoAllocMaxBlocks];
+
+// accumulate_kernel with a fixed range of events per block (the grid, and so the order of the sums, does not
+// depend on the number of SMs).  Every block writes its three entries, also when none of its events passes.
+template <class T>
+__global__ void __launch_bounds__(256) accumulate_noalloc_kernel(const T* __restrict__ me2, const T* __restrict__ wps,
+                                                                 const uint8_t* __restrict__ pass, int64_t n,
+                                                                 double wscale, double* __restrict__ partials) {
+  __shared__ double sh[3][8];
+  double sw = 0, sw2 = 0, np = 0;
+  const int64_t e0 = (int64_t)blockIdx.x * kNoAllocRange;
+  const int64_t e1 = e0 + kNoAllocRange < n ? e0 + kNoAllocRange : n;
+  for (int64_t e = e0 + threadIdx.x; e < e1; e += 256) {
+    const bool ok = pass ? pass[e] != 0 : true;
+    if (ok) {
+      const double w = (double)me2[e] * (double)wps[e] * wscale;
+      sw += w;
+      sw2 += w * w;
+      np += 1.0;
+    }
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    sw += __shfl_down_sync(0xffffffffu, sw, o);
+    sw2 += __shfl_down_sync(0xffffffffu, sw2, o);
+    np += __shfl_down_sync(0xffffffffu, np, o);
+  }
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  if (lane == 0) {
+    sh[0][w] = sw;
+    sh[1][w] = sw2;
+    sh[2][w] = np;
+  }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double a = 0, b = 0, c = 0;
+    for (int i = 0; i < 8; ++i) {
+      a += sh[0][i];
+      b += sh[1][i];
+      c += sh[2][i];
+    }
+    partials[3 * blockIdx.x] = a;
+    partials[3 * blockIdx.x + 1] = b;
+    partials[3 * blockIdx.x + 2] = c;
+  }
+}
+// finalize_kernel writing all four entries of acc to device memory (nb == 0: zeros)
+__global__ void finalize_noalloc_kernel(const double* __restrict__ partials, int nb, int64_t n,
+                                        double* __restrict__ acc) {
+  __shared__ double sh[3][256];
+  double a = 0, b = 0, c = 0;
+  for (int i = threadIdx.x; i < nb; i += blockDim.x) {
+    a += partials[3 * i];
+    b += partials[3 * i + 1];
+    c += partials[3 * i + 2];
+  }
+  sh[0][threadIdx.x] = a;
+  sh[1][threadIdx.x] = b;
+  sh[2][threadIdx.x] = c;
+  __syncthreads();
+  for (int s = blockDim.x / 2; s > 0; s >>= 1) {
+    if ((int)threadIdx.x < s) {
+      sh[0][threadIdx.x] += sh[0][threadIdx.x + s];
+      sh[1][threadIdx.x] += sh[1][threadIdx.x + s];
+      sh[2][threadIdx.x] += sh[2][threadIdx.x + s];
+    }
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) {
+    acc[0] = sh[0][0];
+    acc[1] = sh[1][0];
+    acc[2] = (double)n;
+    acc[3] = sh[2][0];
   }
 }
 
@@ -611,6 +705,62 @@ int hg_accumulate(hg_ctx* ctx, int precision, int64_t n, const void* d_me2, cons
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return fail_cuda(ctx, e, "hg_accumulate");
   return finish(ctx, nblocks, n, acc, s, "hg_accumulate");
+}
+
+// Device address of hg_noalloc_partials on the current device: looked up once per device, with that device
+// current (the symbol has one instance per device).  No allocation.
+static int noalloc_scratch(double** out) {
+  static std::mutex mu;
+  static double* ptr[kNoAllocMaxDevices] = {};
+  int dev = -1;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return fail_cuda_noctx(e, "hg_accumulate_noalloc: cudaGetDevice");
+  if (dev < 0 || dev >= kNoAllocMaxDevices) return fail_noctx(HG_EINVAL, "hg_accumulate_noalloc: device index out of range");
+  std::lock_guard<std::mutex> lock(mu);
+  if (!ptr[dev]) {
+    double* p = nullptr;
+    e = cudaGetSymbolAddress((void**)&p, hg_noalloc_partials);
+    if (e != cudaSuccess) return fail_cuda_noctx(e, "hg_accumulate_noalloc: cudaGetSymbolAddress");
+    if (!p) return fail_noctx(HG_ECUDA, "hg_accumulate_noalloc: cudaGetSymbolAddress returned NULL");
+    ptr[dev] = p;
+  }
+  *out = ptr[dev];
+  return HG_OK;
+}
+
+int hg_accumulate_noalloc(int precision, int64_t n, const void* d_me2, const void* d_wps, const uint8_t* d_pass,
+                          double sqrt_s_hat, double* d_acc, void* cuda_stream) {
+  if (precision != HG_F64 && precision != HG_F32) return fail_noctx(HG_EINVAL, "hg_accumulate_noalloc: unknown precision");
+  if (n < 0) return fail_noctx(HG_EINVAL, "hg_accumulate_noalloc: n < 0");
+  if (n > (int64_t)HG_NOALLOC_MAX_EVENTS)
+    return fail_noctx(HG_EINVAL, "hg_accumulate_noalloc: n exceeds HG_NOALLOC_MAX_EVENTS (16777216 events: the static "
+                                 "scratch array holds 4096 blocks of 4096 events); split the batch");
+  if (!d_acc) return fail_noctx(HG_EINVAL, "hg_accumulate_noalloc: d_acc is NULL");
+  if (misaligned(d_acc, 8)) return fail_noctx(HG_EINVAL, "hg_accumulate_noalloc: misaligned d_acc");
+  if (!finite_pos(sqrt_s_hat)) return fail_noctx(HG_EINVAL, "hg_accumulate_noalloc: sqrt_s_hat must be finite and > 0");
+  if (n > 0 && (!d_me2 || !d_wps)) return fail_noctx(HG_EINVAL, "hg_accumulate_noalloc: d_me2 / d_wps is NULL");
+  if (misaligned(d_me2, precision == HG_F64 ? 8 : 4) || misaligned(d_wps, precision == HG_F64 ? 8 : 4))
+    return fail_noctx(HG_EINVAL, "hg_accumulate_noalloc: misaligned pointer");
+  double* scratch = nullptr;
+  const int rc = noalloc_scratch(&scratch);
+  if (rc != HG_OK) return rc;
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  const double wscale = kHbarC2Pb / (2.0 * sqrt_s_hat * sqrt_s_hat);
+  const int nblocks = (int)((n + kNoAllocRange - 1) / kNoAllocRange);   // <= kNoAllocMaxBlocks
+  if (nblocks > 0) {
+    if (precision == HG_F64)
+      accumulate_noalloc_kernel<double><<<nblocks, 256, 0, s>>>((const double*)d_me2, (const double*)d_wps, d_pass, n,
+                                                                wscale, scratch);
+    else
+      accumulate_noalloc_kernel<float><<<nblocks, 256, 0, s>>>((const float*)d_me2, (const float*)d_wps, d_pass, n,
+                                                               wscale, scratch);
+    const cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail_cuda_noctx(e, "hg_accumulate_noalloc: accumulate_noalloc_kernel");
+  }
+  finalize_noalloc_kernel<<<1, 256, 0, s>>>(scratch, nblocks, n, d_acc);
+  const cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return fail_cuda_noctx(e, "hg_accumulate_noalloc: finalize_noalloc_kernel");
+  return HG_OK;
 }
 
 int hg_integrate_step(hg_ctx* ctx, int process, int precision, uint64_t seed, uint64_t first_event, int64_t n,
