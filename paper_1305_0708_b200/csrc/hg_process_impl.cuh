@@ -27,15 +27,19 @@ namespace hg {
 // by the generator (SmemStage::own), results meeting in the staging area at the next rendezvous.  Two warps per scheduler are what hides the instruction-fetch
 // stall at every 128-byte line of the 170 KB straight-line code (profiles/r01_notes.md section 3).
 constexpr int kSmemPerSM = 227 * 1024;
+// P::n_split == 4 (group split, W + 4 jets): a TEAM of four warps per 32 events, warp t of the team = (half t & 1,
+// group t >> 1): each half of the innermost loop is evaluated by two warps that share out its closings.
 template <class P>
-constexpr int kSplit = P::n_stage > 0 ? 2 : 1;
+constexpr int kSplit = P::n_stage > 0 ? P::n_split : 1;
 constexpr int kGlobalStageThreads = 256;   // global staging area: 4 pairs per block walk the code together
 template <class P, class T>
 constexpr int stage_threads(int want) {
   if (P::n_stage == 0) return want;
   if (P::stage_global) return kGlobalStageThreads;
-  // 32-event groups that fit on an SM, leaving 3 KB for the kernels' static shared memory
-  const int groups = (kSmemPerSM - 3072) / (P::n_stage * (int)sizeof(T) * 32);
+  // 32-event groups that fit on an SM, leaving room for the kernels' static shared memory (3 KB; a team of four
+  // has comb of me2_event, 3 x EPB words, and the scratch of block_reduce3, 384 bytes: at most 1152 bytes)
+  const int groups = (kSmemPerSM - (P::n_split == 4 ? 1152 : 3072)) / (P::n_stage * (int)sizeof(T) * 32);
+  if (P::n_split == 4) return 128 * (groups >= 2 ? 2 : 1);   // one or two teams = 4 or 8 warps
   // 2, 4 or 6 pairs = 4, 8 or 12 warps: a multiple of the 4 schedulers (6 and 10 warps measured slower than 4 and 8)
   const int g = groups >= 6 ? 6 : (groups >= 4 ? 4 : (groups >= 2 ? 2 : 1));
   return 64 * g;
@@ -47,12 +51,12 @@ constexpr size_t stage_bytes() {
 // index of this thread's event within the block, and whether this thread owns the event's result
 template <class P>
 __device__ __forceinline__ int ev_local() {
-  if constexpr (P::n_stage > 0) return ((threadIdx.x >> 6) << 5) | (threadIdx.x & 31);
+  if constexpr (P::n_stage > 0) return ((threadIdx.x / (32 * kSplit<P>)) << 5) | (threadIdx.x & 31);
   return threadIdx.x;
 }
 template <class P>
 __device__ __forceinline__ bool ev_owner() {
-  if constexpr (P::n_stage > 0) return ((threadIdx.x >> 5) & 1) == 0;
+  if constexpr (P::n_stage > 0) return ((threadIdx.x >> 5) % kSplit<P>) == 0;
   return true;
 }
 
@@ -62,22 +66,27 @@ __device__ __forceinline__ bool ev_owner() {
 template <class P, class T, int THREADS>
 __device__ __forceinline__ T me2_event(const Mom<T>* q, const Coup<T>& c, T* gstage) {
   if constexpr (P::n_stage > 0) {
-    constexpr int EPB = THREADS / 2;
+    constexpr int S = kSplit<P>;
+    constexpr int EPB = THREADS / S;
     extern __shared__ __align__(16) unsigned char hg_stage_smem[];
-    __shared__ T comb[EPB];
+    __shared__ T comb[S - 1][EPB];
     const int ev = ev_local<P>();
-    const int half = (threadIdx.x >> 5) & 1;
+    const int wt = (threadIdx.x >> 5) % S;     // warp of the pair / team
+    const int half = wt & 1, group = wt >> 1;
     T r;
     if constexpr (P::stage_global) {
       const GmemStage<T, EPB> st{gstage + (int64_t)blockIdx.x * (P::n_stage * EPB) + ev, half};
       r = P::template me2<T>(q, c, st);
     } else {
-      const SmemStage<T, EPB> st{reinterpret_cast<T*>(hg_stage_smem) + ev, half};
+      const SmemStage<T, EPB> st{reinterpret_cast<T*>(hg_stage_smem) + ev, half, group};
       r = P::template me2<T>(q, c, st);
     }
-    if (half) comb[ev] = r;
+    if (wt) comb[wt - 1][ev] = r;
     __syncthreads();
-    if (!half) r += comb[ev];
+    if (!wt) {
+#pragma unroll
+      for (int i = 0; i < S - 1; ++i) r += comb[i][ev];   // fixed order: deterministic
+    }
     __syncthreads();  // comb and the staging area are free for the next event
     return r;
   } else {
@@ -153,7 +162,7 @@ __global__ void __launch_bounds__(128) ps_kernel(const PsConst k, uint64_t seed,
 
 // Block reduction of three doubles: warp shuffle, then one value per warp through shared memory.
 __device__ __forceinline__ void block_reduce3(double& a, double& b, double& c) {
-  __shared__ double sh[3][32];
+  __shared__ double sh[3][16];   // up to 12 warps per block (stage_threads)
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) {
     a += __shfl_down_sync(0xffffffffu, a, o);
@@ -340,7 +349,7 @@ struct Launch {
       if (err != cudaSuccess) return err;
       const int per_sm = a < b ? a : b;
       *blocks = n_sm * (per_sm < 1 ? 1 : per_sm);
-      *bytes = (size_t)*blocks * (TH / 2) * P::n_stage * sizeof(T);
+      *bytes = (size_t)*blocks * (TH / kSplit<P>) * P::n_stage * sizeof(T);
     }
     return cudaSuccess;
   }

@@ -23,10 +23,13 @@ template <class T, int STRIDE>
 struct SmemStage {
   T* b;      // shared memory + index of the event in the block
   int half;  // which half of the innermost helicity loop this warp evaluates (pair split, hg_process_impl.cuh)
+  int group; // which group of closings of the innermost loop body (group split, P::n_split == 4; else 0)
   __device__ __forceinline__ int lo() const { return half; }
   __device__ __forceinline__ int hi() const { return half + 1; }
   // does this warp evaluate the part of a shared phase dealt to half h? (emit.py _render_shared)
-  __device__ __forceinline__ bool own(int h) const { return half == h; }
+  __device__ __forceinline__ bool own(int h) const { return half == h && group == 0; }
+  // does this warp evaluate group g of the closings of the innermost loop body? (emit.py _partition)
+  __device__ __forceinline__ bool grp(int g) const { return group == g; }
   __device__ __forceinline__ T get(int s) const { return ((volatile T*)b)[s * STRIDE]; }
   __device__ __forceinline__ void put(int s, T v) const { b[s * STRIDE] = v; }
   // Block-wide rendezvous, emitted by the generator at the top of every helicity-loop iteration: the two warps of
@@ -49,6 +52,7 @@ struct GmemStage {
   __device__ __forceinline__ int lo() const { return half; }
   __device__ __forceinline__ int hi() const { return half + 1; }
   __device__ __forceinline__ bool own(int h) const { return half == h; }
+  __device__ __forceinline__ bool grp(int) const { return true; }   // pairs only: a warp runs every group in turn
   __device__ __forceinline__ T get(int s) const { return ((volatile T*)b)[s * STRIDE]; }
   __device__ __forceinline__ void put(int s, T v) const { ((volatile T*)b)[s * STRIDE] = v; }
   __device__ __forceinline__ void sync() const { __syncthreads(); }   // also orders the block's global accesses
@@ -62,6 +66,7 @@ struct HostStage {
   int lo() const { return 0; }
   int hi() const { return 2; }
   bool own(int) const { return true; }
+  bool grp(int) const { return true; }
   void sync() const {}
 };
 
@@ -140,6 +145,41 @@ HG_HD void acc_add(const St& st, int s, T k, cx<T> rb, cx<T> ib) {
   st.put(s + 1, st.get(s + 1) + k * rb.im);
   st.put(s + 2, st.get(s + 2) + k * ib.re);
   st.put(s + 3, st.get(s + 3) + k * ib.im);
+}
+// Op calls (gen/emit.py, option opcalls): the generated op functions of a process are REAL functions on the device
+// (arguments and results by value: the ABI keeps them in registers), so that the innermost loop body is a sequence
+// of short call sites instead of hundreds of KB of inlined arithmetic.
+#if defined(__CUDACC__)
+#define HG_OPCALL __host__ __device__ __noinline__
+#else
+#define HG_OPCALL inline
+#endif
+// what a closing returns: the projections on eps(+1) of the closing leg and on its conjugate (hg_helas.cuh close_proj)
+template <class T>
+struct RbIb {
+  cx<T> rb, ib;
+};
+// the non-zero half of a single-chirality spinor (slot mask M = SLOT_A or SLOT_B): what an op function passes
+template <class T>
+struct Sh {
+  cx<T> c[2];
+};
+template <int M, class T>
+HG_HD Sh<T> sp_half(const Sp<T>& f) {
+  constexpr int o = (M & SLOT_A) ? 0 : 2;
+  Sh<T> h;
+  h.c[0] = f.c[o];
+  h.c[1] = f.c[o + 1];
+  return h;
+}
+template <int M, class T>
+HG_HD Sp<T> sp_full(const Sh<T>& h) {
+  constexpr int o = (M & SLOT_A) ? 0 : 2;
+  Sp<T> f;
+  for (int i = 0; i < 4; ++i) f.c[i] = czero<T>();
+  f.c[o] = h.c[0];
+  f.c[o + 1] = h.c[1];
+  return f;
 }
 // polarisation vector of a massless vector leg, helicity +1: eps^0 = 0 and eps^3 is real, so 5 words.
 // flip != 0 returns the helicity -1 vector -conj(eps) (vflip).

@@ -205,12 +205,24 @@ class CodeGen(Emitter):
     # 1.5 % faster, the fused fp32 step of W + 2 jets 15 % slower)
     POL_LC = True
 
-    def __init__(self, diag, stage=False, kfromp=False, dress=None):
+    def __init__(self, diag, stage=False, kfromp=False, dress=None, groups=1, opcalls=False):
         super().__init__(diag)
         if dress is not None:
             self.DRESS = dress
         self.stage = stage
         self.kfromp = stage and kfromp   # inside loops rebuild internal momenta from staged external momenta
+        # group split (staged processes with the accumulators in the staging area): the closings of the innermost
+        # loop body are dealt to `groups` warps (with the currents each needs; a current two groups need is
+        # evaluated by both), each with its own set of accumulators, so that a TEAM of 2 x groups warps evaluates an
+        # event; the colour contraction adds the sets up, one helicity of the closing leg per group.
+        self.groups = groups if stage else 1
+        # op calls (staged processes with the accumulators in the staging area): the arithmetic of every vertex call
+        # of the innermost loop body becomes a call of a REAL function, one per distinct shape of call (routine,
+        # template arguments, kinds of operands); operands and results travel by value (the ABI keeps them in
+        # registers) and the loads from the staging area stay at the call site.  The inlined body of W + 4 jets is
+        # 600 KB of SASS, far beyond the instruction caches, and with one warp per scheduler nothing hides the
+        # fetch latency; a dozen arithmetic-only functions stay cached (DESIGN.md section 9 NEXT-4).
+        self.opcalls = stage and opcalls
 
     # ------------------------------------------------------------------ value registry / operand access
     def _reg(self, name, ctype, depth, mask=AB, region=None, pol_of=None, hvar=None):
@@ -289,6 +301,8 @@ class CodeGen(Emitter):
         self.need_ratio = set()   # ratios of couplings 'r_<coupling>_mgs'
         self.shared = {}          # key -> name of depth-0 values already emitted
         self.shared_items = []
+        self.op_funcs = {}        # shape -> name of the op function
+        self.prelude = []         # lines emitted before the me2 function (the op functions)
         dyn = self.dynamic
         self.depth_of_leg = {l: i + 1 for i, l in enumerate(dyn)}
         for l in dyn:
@@ -413,6 +427,114 @@ class CodeGen(Emitter):
                 _, lines, loads = it
                 out.append(ind + '{ ' + ' '.join(loads))
                 for ln in lines:
+                    out.append(ind + '  ' + ln)
+                out.append(ind + '}')
+        return out
+
+    # ------------------------------------------------------------------ op calls (innermost loop body)
+    _RE_REG = re.compile(r'\b(v\d+_\d+|[xya]\d+)\b')
+    _RE_CPL = re.compile(r'\bc\.\w+\b')
+    _RE_ACC = re.compile(r'acc_add<T>\(st, A \+ (\d+), T\((-?\d+)\), rb, ib\);$')
+    _RE_ALIAS = re.compile(r'^const ([A-Za-z]+(?:<T>)?) (a\d+) = (\w+)(?:<(\d), T>)?')
+
+    def _reg_ctype(self, name):
+        if name[0] == 'y':
+            return 'Pol<T>'
+        if name[0] == 'x':
+            return 'Vc<T>'
+        v = self.vals[name]
+        return 'Vc<T>' if v['ctype'] == 'pol' else v['ctype']
+
+    def _op_call(self, ret, loads, body, ret_mask=AB):
+        """Call expression of the op function with the shape of `body` (created on first use).  Couplings become T
+        parameters (one per occurrence), register operands and the aliases of `loads` by-value parameters (one per
+        distinct operand); a single-chirality spinor travels as its non-zero half (hg_stage.cuh Sh<T>)."""
+        params, args, regs, unpack = [], [], {}, []
+        count = {'g': 0, 'r': 0}
+        alias = {}
+        for ln in loads:
+            m = self._RE_ALIAS.match(ln)
+            assert m, ln
+            alias[m.group(2)] = (m.group(1), int(m.group(4)) if m.group(3) == 'ld_sp' else AB)
+
+        def param(kind, ctype, actual):
+            if kind == 'r' and actual in regs:
+                return regs[actual]
+            pname = '%s%d' % (kind, count[kind])
+            count[kind] += 1
+            m = AB
+            if kind == 'r' and ctype == 'Sp<T>':
+                m = alias[actual][1] if actual in alias else self.vals[actual]['mask']
+            if m != AB:
+                params.append('Sh<T> %sh' % pname)
+                args.append('sp_half<%d>(%s)' % (m, actual))
+                unpack.append('const Sp<T> %s = sp_full<%d>(%sh);' % (pname, m, pname))
+            else:
+                params.append('%s %s' % (ctype, pname))
+                args.append(actual)
+            if kind == 'r':
+                regs[actual] = pname
+            return pname
+
+        def ctype_of(name):
+            return alias[name][0] if name in alias else self._reg_ctype(name)
+
+        out = []
+        for ln in body:
+            assert '(st' not in ln, ln
+            ln = self._RE_REG.sub(lambda m: param('r', ctype_of(m.group(1)), m.group(1)), ln)
+            ln = self._RE_CPL.sub(lambda m: param('g', 'T', m.group(0)), ln)
+            out.append(ln)
+        out = unpack + out
+        half = None
+        if ret == 'Sp<T>' and ret_mask != AB:
+            half = ret_mask
+            ret = 'Sh<T>'
+            assert out[-1].startswith('return ')
+            out[-1] = 'return sp_half<%d>(%s);' % (half, out[-1][len('return '):-1])
+        key = (ret, tuple(params), tuple(out))
+        if key not in self.op_funcs:
+            name = 'op_%s_%d' % (self.dg.spec.name, len(self.op_funcs))
+            self.op_funcs[key] = name
+            self.prelude.append('template <class T>')
+            self.prelude.append('HG_OPCALL %s %s(%s) {' % (ret, name, ', '.join(params)))
+            self.prelude += ['  ' + ln for ln in out]
+            self.prelude.append('}')
+        call = '%s<T>(%s)' % (self.op_funcs[key], ', '.join(args))
+        return 'sp_full<%d>(%s)' % (half, call) if half else call
+
+    def _render_calls(self, items, ind):
+        """The innermost loop body with the arithmetic of every vertex call in an op function (see __init__)."""
+        out = []
+        for it in items:
+            if it[0] == 'raw':
+                out.append(ind + it[1])
+            elif it[0] == 'def':
+                _, name, expr, loads = it
+                v = self.vals[name]
+                ct = 'Vc<T>' if v['ctype'] == 'pol' else v['ctype']
+                if '(' not in expr:          # a sum of register values: stays in line
+                    assert not loads
+                    out.append(ind + 'const %s %s = %s;' % (ct, name, expr))
+                else:
+                    call = self._op_call(ct, loads, ['return %s;' % expr], v['mask'])
+                    if loads:
+                        out.append(ind + '%s %s;' % (ct, name))
+                        out.append(ind + '{ ' + ' '.join(loads))
+                        out.append(ind + '  %s = %s; }' % (name, call))
+                    else:
+                        out.append(ind + 'const %s %s = %s;' % (ct, name, call))
+                if v['slot'] is not None:
+                    out.append(ind + self._store_line(v))
+            else:
+                _, lines, loads = it
+                work = [ln for ln in lines if not self._RE_ACC.match(ln)]
+                accs = [ln for ln in lines if self._RE_ACC.match(ln)]
+                assert accs and len(work) + len(accs) == len(lines), lines
+                call = self._op_call('RbIb<T>', loads, work + ['return RbIb<T>{rb, ib};'])
+                out.append(ind + '{ ' + ' '.join(loads))
+                out.append(ind + '  const RbIb<T> q = %s; const cx<T> rb = q.rb, ib = q.ib;' % call)
+                for ln in accs:
                     out.append(ind + '  ' + ln)
                 out.append(ind + '}')
         return out
@@ -730,9 +852,11 @@ class CodeGen(Emitter):
         # Many colour flows (W + 4 jets: 24): the 2 nf complex accumulators would take 8 nf registers of fp64, so
         # they live in the staging area instead, one set per warp of the pair.
         acc_smem = cbc and self.stage and nf > self.ACC_IN_REGS_MAX
+        G = self.groups if acc_smem else 1
+        assert G in (1, 2)
         if acc_smem:
             accbase = self.n_slots[1]
-            self.n_slots[1] += 8 * nf
+            self.n_slots[1] += 8 * nf * G
             self.max_slots[1] = max(self.max_slots[1], self.n_slots[1])
         for rt in roots:
             for ch in rt.children:
@@ -768,13 +892,21 @@ class CodeGen(Emitter):
                     else:
                         lines.append('j%d = j%d + T(%d) * a;' % (f, f, cf))
             inner.append(('blk', lines, self.cur_loads))
+        if G == 2:
+            levels[k] = inner = [('grp', self._partition(inner))]
         # colour contraction (symmetric form)
         tail = []
         if cbc:
             tail.append('#pragma unroll')
             tail.append('for (int h%d = 0; h%d < 2; ++h%d) {' % (last, last, last))
             tail.append('  const T sg = h%d ? T(-1) : T(1);' % last)
-            if acc_smem:
+            if acc_smem and G == 2:
+                o = 4 * nf
+                tail.append('  const cx<T> ' + ', '.join(
+                    'j%d = close_amp(ld_cx<T>(st, A + %d) + ld_cx<T>(st, A + %d), ld_cx<T>(st, A + %d) + '
+                    'ld_cx<T>(st, A + %d), sg)' % (f, 4 * f, o + 4 * f, 4 * f + 2, o + 4 * f + 2)
+                    for f in range(nf)) + ';')
+            elif acc_smem:
                 tail.append('  const cx<T> ' + ', '.join(
                     'j%d = close_amp(ld_cx<T>(st, A + %d), ld_cx<T>(st, A + %d), sg)' % (f, 4 * f, 4 * f + 2)
                     for f in range(nf)) + ';')
@@ -791,7 +923,15 @@ class CodeGen(Emitter):
                 terms.append('T(%d) * j%d' % (cval, g))
             tail.append(pre + '{ const cx<T> t = %s; me += j%d.re * t.re + j%d.im * t.im; }' % (
                 ' + '.join(terms), f, f))
-        if cbc and acc_smem:
+        if cbc and acc_smem and G == 2:
+            # the sets of the two groups are complete after a rendezvous of the team; group g contracts helicity g
+            tail[0] = '#pragma unroll 1'
+            tail[1] = 'for (int h%d = 0; h%d < 2; ++h%d) if (st.grp(h%d)) {' % (last, last, last, last)
+            tail.append('}')
+            tail = ['st.sync();', 'const int A = L + %d + st.lo() * %d;' % (accbase, 8 * nf)] + tail
+            accdecl = ('const int A = L + %d + (st.lo() * 2 + %%d) * %d; for (int i = 0; i < %d; ++i) '
+                       'st.put(A + i, T(0));' % (accbase, 4 * nf, 4 * nf))
+        elif cbc and acc_smem:
             tail.append('}')
             accdecl = ('const int A = L + %d + st.lo() * %d; for (int i = 0; i < %d; ++i) st.put(A + i, T(0));'
                        % (accbase, 4 * nf, 4 * nf))
@@ -800,7 +940,46 @@ class CodeGen(Emitter):
             accdecl = 'cx<T> ' + ', '.join('X%d = czero<T>(), Y%d = czero<T>()' % (f, f) for f in range(nf)) + ';'
         else:
             accdecl = 'cx<T> ' + ', '.join('j%d = czero<T>()' % f for f in range(nf)) + ';'
-        return dict(hel=hel, levels=levels, tail=tail, k=k, accdecl=accdecl)
+        return dict(hel=hel, levels=levels, tail=tail, k=k, accdecl=accdecl, groups=G,
+                    calls=bool(cbc and acc_smem and self.opcalls))
+
+    def _partition(self, inner):
+        """Deals the closings ('blk' items) of the innermost loop body to two groups, each with the 'def' items its
+        closings need (in the original order).  Greedy, in order (neighbouring closings share currents): a closing
+        goes to the group whose estimated cost grows less, with the running totals as the balance."""
+        index = {it[1]: i for i, it in enumerate(inner) if it[0] == 'def'}
+        deps, cost = [], []
+        for i, it in enumerate(inner):
+            text = it[2] if it[0] == 'def' else ' '.join(it[1])
+            deps.append({index[n] for n in re.findall(r'v\d+_\d+', text) if n in index and index[n] != i})
+            c = 8
+            for fn, w in self._CALL_COST:
+                if fn in text:
+                    c = w
+                    break
+            cost.append(c + 4 * text.count('acc_add'))
+        memo = {}
+
+        def closure(i):
+            if i not in memo:
+                r = {i}
+                for j in deps[i]:
+                    r |= closure(j)
+                memo[i] = r
+            return memo[i]
+
+        have, total = [set(), set()], [0, 0]
+        for i, it in enumerate(inner):
+            if it[0] != 'blk':
+                continue
+            need = closure(i)
+            add = [sum(cost[j] for j in need - have[g]) for g in (0, 1)]
+            g = 0 if total[0] + add[0] <= total[1] + add[1] else 1
+            have[g] |= need
+            total[g] += add[g]
+        assert all(i in have[0] or i in have[1] for i in range(len(inner)))
+        self.group_cost = total
+        return [[inner[i] for i in sorted(h)] for h in have]
 
     def _dressed_closing(self, rt, vi, hel, k):
         """Lines that compute rb, ib of an FFV root as spinor dot products, or None if neither spinor is helicity-loop
@@ -870,9 +1049,20 @@ class CodeGen(Emitter):
             if self.stage:
                 b.append(ind + 'st.sync();')
             b.append(ind + self._dyn_leaf_decl(lg))
-            if d == k:
+            render = self._render_calls if var['calls'] else self._render_items
+            if d == k and var['groups'] == 2:
+                for g, items in enumerate(levels[d][0][1]):
+                    b.append(ind + 'if (st.grp(%d)) {  // estimated %d flops' % (g, self.group_cost[g]))
+                    b.append(ind + '  ' + var['accdecl'] % g)
+                    body = render(items, ind + '  ')
+                    assert not any('st.sync' in ln for ln in body), 'block barrier under st.grp()'
+                    b += body
+                    b.append(ind + '}')
+            elif d == k:
                 b.append(ind + var['accdecl'])
-            b += self._render_items(levels[d], ind) if d == k else self._render_shared(levels[d], ind)
+                b += render(levels[d], ind)
+            else:
+                b += self._render_shared(levels[d], ind)
         for line in var['tail']:
             b.append(ind + line)
         for d in range(k):

@@ -89,6 +89,13 @@ NO_DRESS = {4}
 # through shared memory, 34.9 ms against 26.5 ms per 2^18 events in fp64, 27.2 against 12.9 ms in fp32, whether the
 # 8 warps sit in one block or four (profiles/r02_notes.md): the option stays off.
 STAGE_GLOBAL = set()
+# staged processes evaluated by a TEAM of four warps per 32 events: the closings of the innermost loop body are dealt
+# to two groups of warps (gen/emit.py groups).  W + 4 jets keeps 711 words per event, i.e. one pair of warps per SM in
+# fp64 with two of the four schedulers idle; the second set of accumulators (+192 words) still fits
+GROUPS = {9: 2}
+# staged processes whose innermost loop body calls one real function per shape of vertex call instead of inlining
+# the arithmetic of every call (gen/emit.py opcalls)
+OPCALLS = set()
 
 
 def build(spec, last=None):
@@ -98,7 +105,7 @@ def build(spec, last=None):
         last = spec.last
     def make(leg):
         cg_ = CodeGen(Diagrams(spec, merge=MERGE).build(leg), stage, spec.pid in KFROMP,
-                      dress=spec.pid not in NO_DRESS)
+                      dress=spec.pid not in NO_DRESS, groups=GROUPS.get(spec.pid, 1), opcalls=spec.pid in OPCALLS)
         cg_.count_dg = Diagrams(spec).build(leg)   # Feynman-diagram counts: the unmerged enumeration
         return cg_
 
@@ -134,6 +141,7 @@ def render(cg):
         '#include "../hg_params.cuh"',
         '#include "../hg_stage.cuh"',
         'namespace hg {',
+    ] + list(cg.prelude) + [
         'template <class T, class St>',
         'HG_HD T me2_%s(const Mom<T>* p, const Coup<T>& c, const St& st) {' % spec.name,
     ]
@@ -212,6 +220,7 @@ struct P%(pid)d {
   static constexpr int n_draws = %(n_draws)d;
   static constexpr int n_stage = %(n_stage)d;  // words per event of the staging area (0: not staged)
   static constexpr bool stage_global = %(stage_global)s;  // the staging area is global memory, not shared
+  static constexpr int n_split = %(n_split)d;  // warps that share an event of a staged process: pair, or team of four
   // hg_integrate_step as phase-space kernel + compaction + |M|^2 kernel per chunk (true) or one fused kernel
   static constexpr bool split_step = %(split_step)s;
   static constexpr double avg_factor = %(avg)s;
@@ -247,6 +256,7 @@ struct P%(pid)d {
            n_hel_nonzero=row['n_hel_nonzero'], n_diagrams=row['n_diagrams'], n_amplitudes=row['n_amplitudes'],
            n_flows=row['n_flows'], n_draws=row['n_draws'], n_stage=cg.n_stage,
            stage_global='true' if spec.pid in STAGE_GLOBAL else 'false',
+           n_split=2 * GROUPS.get(spec.pid, 1),
            split_step='true' if (cg.n_stage > 0 or spec.pid in SPLIT_STEP) else 'false', avg=repr(row['avg_factor']),
            me_threads=ME_THREADS.get(spec.pid, 128), n_jets=len(jets), n_leps=len(leps), jets=arr(jets),
            leps=arr(leps), gen_call=gen_call, has_had='true' if had_call else 'false',
