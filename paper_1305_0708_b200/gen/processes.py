@@ -95,7 +95,7 @@ STAGE_GLOBAL = set()
 GROUPS = {9: 2}
 # staged processes whose innermost loop body calls one real function per shape of vertex call instead of inlining
 # the arithmetic of every call (gen/emit.py opcalls)
-OPCALLS = set()
+OPCALLS = {9}
 
 
 def build(spec, last=None):
