@@ -434,7 +434,7 @@ class CodeGen(Emitter):
     # ------------------------------------------------------------------ op calls (innermost loop body)
     _RE_REG = re.compile(r'\b(v\d+_\d+|[xya]\d+)\b')
     _RE_CPL = re.compile(r'\bc\.\w+\b')
-    _RE_ACC = re.compile(r'acc_add<T>\(st, A \+ (\d+), T\((-?\d+)\), rb, ib\);$')
+    _RE_ACC = re.compile(r'^(acc_add<T>\(st, A \+ \d+, T\(-?\d+\), rb, ib\);|X\d+ = X\d+ |j\d+ = j\d+ )')
     _RE_ALIAS = re.compile(r'^const ([A-Za-z]+(?:<T>)?) (a\d+) = (\w+)(?:<(\d), T>)?')
 
     def _reg_ctype(self, name):
@@ -531,9 +531,14 @@ class CodeGen(Emitter):
                 work = [ln for ln in lines if not self._RE_ACC.match(ln)]
                 accs = [ln for ln in lines if self._RE_ACC.match(ln)]
                 assert accs and len(work) + len(accs) == len(lines), lines
-                call = self._op_call('RbIb<T>', loads, work + ['return RbIb<T>{rb, ib};'])
                 out.append(ind + '{ ' + ' '.join(loads))
-                out.append(ind + '  const RbIb<T> q = %s; const cx<T> rb = q.rb, ib = q.ib;' % call)
+                if any(' rb' in ln for ln in work):     # closing by current: projections on eps(+) and its conjugate
+                    call = self._op_call('RbIb<T>', loads, work + ['return RbIb<T>{rb, ib};'])
+                    out.append(ind + '  const RbIb<T> q = %s; const cx<T> rb = q.rb, ib = q.ib;' % call)
+                else:                                   # closing by amplitude
+                    assert len(work) == 1 and work[0].startswith('const cx<T> a = '), work
+                    call = self._op_call('cx<T>', loads, ['return ' + work[0][len('const cx<T> a = '):]])
+                    out.append(ind + '  const cx<T> a = %s;' % call)
                 for ln in accs:
                     out.append(ind + '  ' + ln)
                 out.append(ind + '}')
@@ -941,7 +946,7 @@ class CodeGen(Emitter):
         else:
             accdecl = 'cx<T> ' + ', '.join('j%d = czero<T>()' % f for f in range(nf)) + ';'
         return dict(hel=hel, levels=levels, tail=tail, k=k, accdecl=accdecl, groups=G,
-                    calls=bool(cbc and acc_smem and self.opcalls))
+                    calls=bool(self.opcalls and k > 0))
 
     def _partition(self, inner):
         """Deals the closings ('blk' items) of the innermost loop body to two groups, each with the 'def' items its
