@@ -26,8 +26,8 @@ struct SmemStage {
   int group; // which group of closings of the innermost loop body (group split, P::n_split == 4; else 0)
   __device__ __forceinline__ int lo() const { return half; }
   __device__ __forceinline__ int hi() const { return half + 1; }
-  // does this warp evaluate the part of a shared phase dealt to half h? (emit.py _render_shared)
-  __device__ __forceinline__ bool own(int h) const { return half == h && group == 0; }
+  // does this warp evaluate the part of a shared phase dealt to warp h of the pair / team? (emit.py _render_shared)
+  __device__ __forceinline__ bool own(int h) const { return half + 2 * group == h; }
   // does this warp evaluate group g of the closings of the innermost loop body? (emit.py _partition)
   __device__ __forceinline__ bool grp(int g) const { return group == g; }
   __device__ __forceinline__ T get(int s) const { return ((volatile T*)b)[s * STRIDE]; }

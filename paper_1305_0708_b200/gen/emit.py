@@ -379,15 +379,16 @@ class CodeGen(Emitter):
         groups = {}
         for i in range(len(items)):
             groups.setdefault(find(i), []).append(i)
-        load = [0, 0]
+        nown = 2 * self.groups       # warps that share an event: pair, or team of four
+        load = [0] * nown
         owner = {}
         for root, members in sorted(groups.items(), key=lambda kv: -sum(cost[i] for i in kv[1])):
-            h = 0 if load[0] <= load[1] else 1
+            h = load.index(min(load))
             load[h] += sum(cost[i] for i in members)
             for i in members:
                 owner[i] = h
         out = self._render_items(both, ind)
-        for h in (0, 1):
+        for h in range(nown):
             mine = [items[i] for i in range(len(items)) if owner[i] == h]
             if not mine:
                 continue
@@ -857,8 +858,9 @@ class CodeGen(Emitter):
         # Many colour flows (W + 4 jets: 24): the 2 nf complex accumulators would take 8 nf registers of fp64, so
         # they live in the staging area instead, one set per warp of the pair.
         acc_smem = cbc and self.stage and nf > self.ACC_IN_REGS_MAX
-        G = self.groups if acc_smem else 1
-        assert G in (1, 2)
+        G = self.groups
+        if not (G == 1 or (G == 2 and acc_smem)):
+            raise NotImplementedError('group split needs the accumulators in the staging area (closing by current)')
         if acc_smem:
             accbase = self.n_slots[1]
             self.n_slots[1] += 8 * nf * G
