@@ -39,7 +39,7 @@ constexpr int stage_threads(int want) {
   // 32-event groups that fit on an SM, leaving room for the kernels' static shared memory (3 KB; a team of four
   // has comb of me2_event, 3 x EPB words, and the scratch of block_reduce3, 384 bytes: at most 1152 bytes)
   const int groups = (kSmemPerSM - (P::n_split == 4 ? 1152 : 3072)) / (P::n_stage * (int)sizeof(T) * 32);
-  if (P::n_split == 4) return 128 * (groups >= 2 ? 2 : 1);   // one or two teams = 4 or 8 warps
+  if (P::n_split == 4) return 128 * (groups >= 3 ? 3 : (groups >= 2 ? 2 : 1));   // one to three teams = 4, 8, 12 warps
   // 2, 4 or 6 pairs = 4, 8 or 12 warps: a multiple of the 4 schedulers (6 and 10 warps measured slower than 4 and 8)
   const int g = groups >= 6 ? 6 : (groups >= 4 ? 4 : (groups >= 2 ? 2 : 1));
   return 64 * g;

@@ -867,7 +867,7 @@ class CodeGen(Emitter):
         last = self.dg.last
         # Many colour flows (W + 4 jets: 24): the 2 nf complex accumulators would take 8 nf registers of fp64, so
         # they live in the staging area instead, one set per warp of the pair.
-        acc_smem = cbc and self.stage and nf > self.ACC_IN_REGS_MAX
+        acc_smem = cbc and self.stage and (nf > self.ACC_IN_REGS_MAX or self.groups > 1)
         G = self.groups
         if not (G == 1 or (G == 2 and acc_smem)):
             raise NotImplementedError('group split needs the accumulators in the staging area (closing by current)')
@@ -960,6 +960,9 @@ class CodeGen(Emitter):
         return dict(hel=hel, levels=levels, tail=tail, k=k, accdecl=accdecl, groups=G,
                     calls=bool(self.opcalls and k > 0))
 
+    # (A cost table with the closings' own flops -- jvv_bare 140, jggg_bare 110, ffv_current 80, sdot 32, 8 per
+    # accumulator update -- balances the four warps of W + 4 jets to 2 % instead of 11 % in counted flops but
+    # duplicates more sub-currents: 14.15 -> 14.30 ms in fp64, 5.96 -> 5.80 ms in fp32 per 2^18 events; not adopted.)
     def _partition(self, inner):
         """Deals the closings ('blk' items) of the innermost loop body to two groups, each with the 'def' items its
         closings need (in the original order).  Greedy, in order (neighbouring closings share currents): a closing

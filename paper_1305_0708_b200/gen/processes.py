@@ -92,6 +92,8 @@ STAGE_GLOBAL = set()
 # staged processes evaluated by a TEAM of four warps per 32 events: the closings of the innermost loop body are dealt
 # to two groups of warps (gen/emit.py groups).  W + 4 jets keeps 711 words per event, i.e. one pair of warps per SM in
 # fp64 with two of the four schedulers idle; the second set of accumulators (+192 words) still fits
+# (measured for config 5 too: three teams = 12 warps per SM at 168 registers with the accumulators in the staging area,
+# 9.8 % duplicated sub-currents: |M|^2 of 2^22 events 4.67 -> 7.97 ms in fp64, 2.66 -> 5.29 ms in fp32 -- pairs stay)
 GROUPS = {9: 2}
 # staged processes whose innermost loop body calls one real function per shape of vertex call instead of inlining
 # the arithmetic of every call (gen/emit.py opcalls).  Measured on B200, |M|^2 of 2^22 events (2^18 for W + 4 jets):

@@ -22,7 +22,7 @@ N = {1: 64, 2: 48, 3: 24, 4: 4, 5: 6, 6: 64, 7: 48, 8: 48, 9: 3, 10: 48, 11: 48}
 @pytest.fixture(scope='module')
 def exe(tmp_path_factory):
     out = str(tmp_path_factory.mktemp('hostcheck') / 'hostcheck')
-    subprocess.check_call(['g++', '-O1', '-std=c++17', SRC, '-o', out, '-lm'])
+    subprocess.check_call(['g++', '-O1', '-std=c++17', '-pthread', SRC, '-o', out, '-lm'])
     return out
 
 
@@ -37,6 +37,23 @@ def test_generated_code_matches_oracle(exe, cfg):
     assert got.shape == ref.shape
     rel = np.abs(got - ref) / ref
     assert rel.max() <= 1e-11, (cfg, rel.max())
+
+
+@pytest.mark.parametrize('cfg', [4, 5, 9])
+def test_pair_and_team_execution_matches_oracle(exe, cfg):
+    """The staged matrix elements evaluated the way the kernels do it: by the two warps of a pair (configs 4, 5) or the
+    four warps of a team (W + 4 jets: two halves of the innermost helicity loop x two groups of closings), played by
+    host threads that share one staging area and meet at every st.sync().  Checks what the single-threaded run
+    cannot: the dealing of the shared phases (st.own), the partition of the closings with its duplicated sub-currents
+    (st.grp), the per-warp accumulator sets, and that every rendezvous is reached by every warp."""
+    par = osm.default_params()
+    p, _ = ops.generate(cfg, 9, 0, N[cfg], opr.SQRT_S[cfg], par)
+    ref = opr.me2(opr.config(cfg), p, par)
+    text = '\n'.join('%d ' % cfg + ' '.join('%.17g' % x for x in ev.reshape(-1)) for ev in p) + '\n'
+    out = subprocess.run([exe, 'team'], input=text, capture_output=True, text=True, check=True, timeout=600).stdout.split()
+    got = np.array([float(x) for x in out])
+    assert got.shape == ref.shape
+    assert (np.abs(got - ref) / ref).max() <= 1e-11
 
 
 @pytest.mark.parametrize('cfg', [1, 3, 6, 7, 8, 10, 11])
