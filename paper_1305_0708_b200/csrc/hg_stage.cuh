@@ -181,6 +181,23 @@ HG_HD Sp<T> sp_full(const Sh<T>& h) {
   f.c[o + 1] = h.c[1];
   return f;
 }
+// the same for N flows at once (offsets off[], factors k[]): all 4 N loads first, then the adds and stores, so that
+// one shared-memory latency is paid per batch instead of one per flow
+template <int N, class T, class St>
+HG_HD void acc_add_batch(const St& st, int A, const int (&off)[N], const T (&k)[N], cx<T> rb, cx<T> ib) {
+  T v[4 * N];
+#pragma unroll
+  for (int i = 0; i < N; ++i)
+#pragma unroll
+    for (int j = 0; j < 4; ++j) v[4 * i + j] = st.get(A + off[i] + j);
+#pragma unroll
+  for (int i = 0; i < N; ++i) {
+    st.put(A + off[i], v[4 * i] + k[i] * rb.re);
+    st.put(A + off[i] + 1, v[4 * i + 1] + k[i] * rb.im);
+    st.put(A + off[i] + 2, v[4 * i + 2] + k[i] * ib.re);
+    st.put(A + off[i] + 3, v[4 * i + 3] + k[i] * ib.im);
+  }
+}
 // polarisation vector of a massless vector leg, helicity +1: eps^0 = 0 and eps^3 is real, so 5 words.
 // flip != 0 returns the helicity -1 vector -conj(eps) (vflip).
 template <class T, class St>

@@ -510,6 +510,27 @@ class CodeGen(Emitter):
     # fp64, 5.98 -> 6.26 ms in fp32.
     OP_PREFETCH = False
 
+    # accumulator updates of one closing in batches of this many flows: all loads of a batch are issued before its
+    # first add (acc_add_batch, hg_stage.cuh).  One acc_add per flow left every update waiting for its own
+    # shared-memory load (ncu source view: one DADD per flow with the stall samples of a whole LDS latency).
+    ACC_BATCH = 4
+    _RE_ACC_SMEM = re.compile(r'^acc_add<T>\(st, A \+ (\d+), T\((-?\d+)\), rb, ib\);$')
+
+    def _batch_accs(self, accs):
+        ms = [self._RE_ACC_SMEM.match(ln) for ln in accs]
+        if self.ACC_BATCH < 2 or not all(ms) or len(ms) < 2:
+            return accs
+        out = []
+        for i in range(0, len(ms), self.ACC_BATCH):
+            part = ms[i:i + self.ACC_BATCH]
+            if len(part) == 1:
+                out.append(part[0].group(0))
+                continue
+            out.append('{ const int o[%d] = {%s}; const T k[%d] = {%s}; acc_add_batch<%d, T>(st, A, o, k, rb, ib); }' % (
+                len(part), ', '.join(m.group(1) for m in part), len(part),
+                ', '.join('T(%s)' % m.group(2) for m in part), len(part)))
+        return out
+
     def _render_calls(self, items, ind):
         """The innermost loop body with the arithmetic of every vertex call in an op function (see __init__)."""
         steps = []      # (loads, lines after the loads)
@@ -542,7 +563,8 @@ class CodeGen(Emitter):
                     assert len(work) == 1 and work[0].startswith('const cx<T> a = '), work
                     call = self._op_call('cx<T>', loads, ['return ' + work[0][len('const cx<T> a = '):]])
                     first = 'const cx<T> a = %s;' % ren(call)
-                steps.append(([ren(ln) for ln in loads], ['{ ' + first] + ['  ' + ln for ln in accs] + ['}']))
+                steps.append(([ren(ln) for ln in loads], ['{ ' + first] + ['  ' + ln for ln in self._batch_accs(accs)]
+                              + ['}']))
         out = []
         if not self.OP_PREFETCH:
             for loads, after in steps:
