@@ -513,6 +513,8 @@ class CodeGen(Emitter):
     # accumulator updates of one closing in batches of this many flows: all loads of a batch are issued before its
     # first add (acc_add_batch, hg_stage.cuh).  One acc_add per flow left every update waiting for its own
     # shared-memory load (ncu source view: one DADD per flow with the stall samples of a whole LDS latency).
+    # Measured for W + 4 jets, 2^18 events: one flow at a time 14.15 ms (fp64) / 5.96 ms (fp32), batches of 4
+    # 13.50 / 5.55 ms, batches of 8 13.52 / 5.61 ms.
     ACC_BATCH = 4
     _RE_ACC_SMEM = re.compile(r'^acc_add<T>\(st, A \+ (\d+), T\((-?\d+)\), rb, ib\);$')
 
