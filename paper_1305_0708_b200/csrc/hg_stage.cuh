@@ -19,7 +19,9 @@ namespace hg {
 struct NoStage {};
 
 #if defined(__CUDACC__)
-template <class T, int STRIDE>
+// NAMED: the rendezvous is a named barrier of the warps that share the event (bar.sync id, threads of the pair /
+// team) instead of a block-wide __syncthreads(): pairs and teams of one block no longer wait for each other.
+template <class T, int STRIDE, bool NAMED = false, int TEAM_THREADS = 64>
 struct SmemStage {
   T* b;      // shared memory + index of the event in the block
   int half;  // which half of the innermost helicity loop this warp evaluates (pair split, hg_process_impl.cuh)
@@ -36,7 +38,14 @@ struct SmemStage {
   // a pair share the loop-level slots, so neither may start writing the values of the next iteration while the
   // other still reads those of the current one.  It also keeps the warps of a block close together in the code
   // (shared instruction-cache lines).  Every thread of the block must call me2().
-  __device__ __forceinline__ void sync() const { __syncthreads(); }
+  __device__ __forceinline__ void sync() const {
+    if constexpr (NAMED) {
+      const int id = 1 + (int)(threadIdx.x / TEAM_THREADS);   // barrier 0 is __syncthreads; at most 6 teams per block
+      asm volatile("bar.sync %0, %1;" : : "r"(id), "n"(TEAM_THREADS) : "memory");
+    } else {
+      __syncthreads();
+    }
+  }
 };
 // Staging area in GLOBAL memory (P::stage_global: W + 4 jets, 738 words = 5.9 KB per event in fp64, which in shared
 // memory leaves room for one pair of warps per SM).  Every block of the persistent grid owns a region laid out

@@ -101,6 +101,11 @@ GROUPS = {9: 2}
 #   config 5    fp64  4.60 ->  5.83 ms, fp32 2.66 -> 3.40 ms   (8-12 warps per SM hide it; the calls only cost)
 #   config 4    fp64  4.43 ->  5.02 ms, fp32 2.71 -> 3.20 ms
 OPCALLS = {9}
+# staged processes whose fp64 rendezvous is a named barrier per pair instead of __syncthreads().  bench.py, B200,
+# 2^22 events, step / dominant kernel per 2^20 events: config 5 fp64 5.097 -> 4.978 ms / 1.077 -> 1.047 ms, config 4
+# fp64 5.662 -> 5.539 ms / 1.125 -> 1.100 ms; in fp32 the named barrier is SLOWER (config 5 3.274 -> 3.334 ms,
+# config 4 3.943 -> 4.081 ms), so fp32 keeps __syncthreads (hg_process_impl.cuh me2_event); W + 4 jets: no difference
+NAMED_BARRIER = {4, 5}
 
 
 def build(spec, last=None):
@@ -226,6 +231,7 @@ struct P%(pid)d {
   static constexpr int n_stage = %(n_stage)d;  // words per event of the staging area (0: not staged)
   static constexpr bool stage_global = %(stage_global)s;  // the staging area is global memory, not shared
   static constexpr int n_split = %(n_split)d;  // warps that share an event of a staged process: pair, or team of four
+  static constexpr bool named_barrier = %(named_barrier)s;  // rendezvous per pair / team, not per block (hg_stage.cuh)
   // hg_integrate_step as phase-space kernel + compaction + |M|^2 kernel per chunk (true) or one fused kernel
   static constexpr bool split_step = %(split_step)s;
   static constexpr double avg_factor = %(avg)s;
@@ -262,6 +268,7 @@ struct P%(pid)d {
            n_flows=row['n_flows'], n_draws=row['n_draws'], n_stage=cg.n_stage,
            stage_global='true' if spec.pid in STAGE_GLOBAL else 'false',
            n_split=2 * GROUPS.get(spec.pid, 1),
+           named_barrier='true' if spec.pid in NAMED_BARRIER else 'false',
            split_step='true' if (cg.n_stage > 0 or spec.pid in SPLIT_STEP) else 'false', avg=repr(row['avg_factor']),
            me_threads=ME_THREADS.get(spec.pid, 128), n_jets=len(jets), n_leps=len(leps), jets=arr(jets),
            leps=arr(leps), gen_call=gen_call, has_had='true' if had_call else 'false',
