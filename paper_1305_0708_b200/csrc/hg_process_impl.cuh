@@ -32,13 +32,18 @@ constexpr int kSmemPerSM = 227 * 1024;
 template <class P>
 constexpr int kSplit = P::n_stage > 0 ? P::n_split : 1;
 constexpr int kGlobalStageThreads = 256;   // global staging area: 4 pairs per block walk the code together
+// words per event of the staging area: an even number with the paired fp32 layout (P::stage_pairs, hg_stage.cuh)
+template <class P>
+constexpr int stage_words() {
+  return P::stage_pairs ? ((P::n_stage + 1) & ~1) : P::n_stage;
+}
 template <class P, class T>
 constexpr int stage_threads(int want) {
   if (P::n_stage == 0) return want;
   if (P::stage_global) return kGlobalStageThreads;
   // 32-event groups that fit on an SM, leaving room for the kernels' static shared memory (3 KB; a team of four
   // has comb of me2_event, 3 x EPB words, and the scratch of block_reduce3, 384 bytes: at most 1152 bytes)
-  const int groups = (kSmemPerSM - (P::n_split == 4 ? 1152 : 3072)) / (P::n_stage * (int)sizeof(T) * 32);
+  const int groups = (kSmemPerSM - (P::n_split == 4 ? 1152 : 3072)) / (stage_words<P>() * (int)sizeof(T) * 32);
   if (P::n_split == 4) return 128 * (groups >= 3 ? 3 : (groups >= 2 ? 2 : 1));   // one to three teams = 4, 8, 12 warps
   // 2, 4 or 6 pairs = 4, 8 or 12 warps: a multiple of the 4 schedulers (6 and 10 warps measured slower than 4 and 8)
   const int g = groups >= 6 ? 6 : (groups >= 4 ? 4 : (groups >= 2 ? 2 : 1));
@@ -46,7 +51,7 @@ constexpr int stage_threads(int want) {
 }
 template <class P, class T, int THREADS>
 constexpr size_t stage_bytes() {
-  return P::stage_global ? 0 : (size_t)P::n_stage * sizeof(T) * (THREADS / kSplit<P>);
+  return P::stage_global ? 0 : (size_t)stage_words<P>() * sizeof(T) * (THREADS / kSplit<P>);
 }
 // index of this thread's event within the block, and whether this thread owns the event's result
 template <class P>
@@ -80,8 +85,9 @@ __device__ __forceinline__ T me2_event(const Mom<T>* q, const Coup<T>& c, T* gst
     } else {
       // rendezvous per pair in fp64 only: in fp32 (12 warps per SM) the block-wide barrier, which also keeps the
       // warps on the same instruction-cache lines, measured 2-4 % faster; in fp64 (8-12 warps) 2-3 % slower
-      const SmemStage<T, EPB, P::named_barrier && sizeof(T) == 8, 32 * S> st{reinterpret_cast<T*>(hg_stage_smem) + ev,
-                                                                             half, group};
+      constexpr bool PAIRS = P::stage_pairs && sizeof(T) == 4;   // fp32: complex numbers in one 8-byte access
+      const SmemStage<T, EPB, P::named_barrier && sizeof(T) == 8, 32 * S, PAIRS> st{
+          reinterpret_cast<T*>(hg_stage_smem) + (PAIRS ? 2 * ev : ev), half, group};
       r = P::template me2<T>(q, c, st);
     }
     if (wt) comb[wt - 1][ev] = r;

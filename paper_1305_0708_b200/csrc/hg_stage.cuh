@@ -21,7 +21,10 @@ struct NoStage {};
 #if defined(__CUDACC__)
 // NAMED: the rendezvous is a named barrier of the warps that share the event (bar.sync id, threads of the pair /
 // team) instead of a block-wide __syncthreads(): pairs and teams of one block no longer wait for each other.
-template <class T, int STRIDE, bool NAMED = false, int TEAM_THREADS = 64>
+// PAIRS (fp32 only): the words are laid out [slot / 2][event][slot % 2], so that two consecutive words of an event
+// with an even first slot -- a complex number -- are ONE 8-byte access (get2 / put2).  The fp32 kernels are bound by
+// instruction issue and 16 % of their instructions were 4-byte shared-memory loads.
+template <class T, int STRIDE, bool NAMED = false, int TEAM_THREADS = 64, bool PAIRS = false>
 struct SmemStage {
   T* b;      // shared memory + index of the event in the block
   int half;  // which half of the innermost helicity loop this warp evaluates (pair split, hg_process_impl.cuh)
@@ -32,8 +35,34 @@ struct SmemStage {
   __device__ __forceinline__ bool own(int h) const { return half + 2 * group == h; }
   // does this warp evaluate group g of the closings of the innermost loop body? (emit.py _partition)
   __device__ __forceinline__ bool grp(int g) const { return group == g; }
-  __device__ __forceinline__ T get(int s) const { return ((volatile T*)b)[s * STRIDE]; }
-  __device__ __forceinline__ void put(int s, T v) const { b[s * STRIDE] = v; }
+  __device__ __forceinline__ int at(int s) const { return PAIRS ? (s >> 1) * (2 * STRIDE) + (s & 1) : s * STRIDE; }
+  __device__ __forceinline__ T get(int s) const { return ((volatile T*)b)[at(s)]; }
+  __device__ __forceinline__ void put(int s, T v) const { b[at(s)] = v; }
+  // words s and s + 1
+  __device__ __forceinline__ void get2(int s, T& x, T& y) const {
+    if constexpr (PAIRS) {
+      static_assert(!PAIRS || sizeof(T) == 4, "paired layout: fp32 only");
+      if ((s & 1) == 0) {   // s is a literal in the generated code: the test folds away
+        const unsigned long long u = *(volatile const unsigned long long*)(b + at(s));
+        x = __uint_as_float((unsigned)u);
+        y = __uint_as_float((unsigned)(u >> 32));
+        return;
+      }
+    }
+    x = get(s);
+    y = get(s + 1);
+  }
+  __device__ __forceinline__ void put2(int s, T x, T y) const {
+    if constexpr (PAIRS) {
+      if ((s & 1) == 0) {
+        *(unsigned long long*)(b + at(s)) =
+            (unsigned long long)__float_as_uint(x) | ((unsigned long long)__float_as_uint(y) << 32);
+        return;
+      }
+    }
+    put(s, x);
+    put(s + 1, y);
+  }
   // Block-wide rendezvous, emitted by the generator at the top of every helicity-loop iteration: the two warps of
   // a pair share the loop-level slots, so neither may start writing the values of the next iteration while the
   // other still reads those of the current one.  It also keeps the warps of a block close together in the code
@@ -64,6 +93,8 @@ struct GmemStage {
   __device__ __forceinline__ bool grp(int) const { return true; }   // pairs only: a warp runs every group in turn
   __device__ __forceinline__ T get(int s) const { return ((volatile T*)b)[s * STRIDE]; }
   __device__ __forceinline__ void put(int s, T v) const { ((volatile T*)b)[s * STRIDE] = v; }
+  __device__ __forceinline__ void get2(int s, T& x, T& y) const { x = get(s); y = get(s + 1); }
+  __device__ __forceinline__ void put2(int s, T x, T y) const { put(s, x); put(s + 1, y); }
   __device__ __forceinline__ void sync() const { __syncthreads(); }   // also orders the block's global accesses
 };
 #endif
@@ -72,6 +103,8 @@ struct HostStage {
   T* b;
   T get(int s) const { return b[s]; }
   void put(int s, T v) const { b[s] = v; }
+  void get2(int s, T& x, T& y) const { x = b[s]; y = b[s + 1]; }
+  void put2(int s, T x, T y) const { b[s] = x; b[s + 1] = y; }
   int lo() const { return 0; }
   int hi() const { return 2; }
   bool own(int) const { return true; }
@@ -89,23 +122,25 @@ HG_HD void st_T(const St& st, int s, T v) {
 }
 template <class T, class St>
 HG_HD cx<T> ld_cx(const St& st, int s) {
-  return mk<T>(st.get(s), st.get(s + 1));
+  T re, im;
+  st.get2(s, re, im);
+  return mk<T>(re, im);
 }
 template <class T, class St>
 HG_HD void st_cx(const St& st, int s, cx<T> v) {
-  st.put(s, v.re);
-  st.put(s + 1, v.im);
+  st.put2(s, v.re, v.im);
 }
 template <class T, class St>
 HG_HD Mom<T> ld_mom(const St& st, int s) {
-  return mkmom<T>(st.get(s), st.get(s + 1), st.get(s + 2), st.get(s + 3));
+  T e, x, y, z;
+  st.get2(s, e, x);
+  st.get2(s + 2, y, z);
+  return mkmom<T>(e, x, y, z);
 }
 template <class T, class St>
 HG_HD void st_mom(const St& st, int s, const Mom<T>& v) {
-  st.put(s, v.e);
-  st.put(s + 1, v.x);
-  st.put(s + 2, v.y);
-  st.put(s + 3, v.z);
+  st.put2(s, v.e, v.x);
+  st.put2(s + 2, v.y, v.z);
 }
 template <class T, class St>
 HG_HD Vc<T> ld_vec(const St& st, int s) {
@@ -211,18 +246,16 @@ HG_HD void acc_add_batch(const St& st, int A, const int (&off)[N], const T (&k)[
 // flip != 0 returns the helicity -1 vector -conj(eps) (vflip).
 template <class T, class St>
 HG_HD void st_pol(const St& st, int s, const Vc<T>& e) {
-  st.put(s, e.c[1].re);
-  st.put(s + 1, e.c[1].im);
-  st.put(s + 2, e.c[2].re);
-  st.put(s + 3, e.c[2].im);
+  st.put2(s, e.c[1].re, e.c[1].im);
+  st.put2(s + 2, e.c[2].re, e.c[2].im);
   st.put(s + 4, e.c[3].re);
 }
 template <class T, class St>
 HG_HD Vc<T> ld_pol(const St& st, int s, int flip) {
   Vc<T> v;
   v.c[0] = czero<T>();
-  v.c[1] = mk<T>(st.get(s), st.get(s + 1));
-  v.c[2] = mk<T>(st.get(s + 2), st.get(s + 3));
+  v.c[1] = ld_cx<T>(st, s);
+  v.c[2] = ld_cx<T>(st, s + 2);
   v.c[3] = mk<T>(st.get(s + 4), T(0));
   if (flip) {
     v.c[1].re = -v.c[1].re;
@@ -239,7 +272,8 @@ struct Pol;
 template <class T, class St>
 HG_HD Pol<T> ld_pol_lc(const St& st, int s, int flip) {
   const T sg = flip ? T(-1) : T(1);
-  const T v1r = sg * st.get(s), v1i = st.get(s + 1), v2r = sg * st.get(s + 2), v2i = st.get(s + 3);
+  const cx<T> e1 = ld_cx<T>(st, s), e2 = ld_cx<T>(st, s + 2);
+  const T v1r = sg * e1.re, v1i = e1.im, v2r = sg * e2.re, v2i = e2.im;
   Pol<T> p;
   p.v3 = sg * st.get(s + 4);
   p.ur = mk<T>(v1r + v2i, v1i - v2r);

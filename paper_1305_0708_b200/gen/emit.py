@@ -205,7 +205,7 @@ class CodeGen(Emitter):
     # 1.5 % faster, the fused fp32 step of W + 2 jets 15 % slower)
     POL_LC = True
 
-    def __init__(self, diag, stage=False, kfromp=False, dress=None, groups=1, opcalls=False):
+    def __init__(self, diag, stage=False, kfromp=False, dress=None, groups=1, opcalls=False, align_pairs=False):
         super().__init__(diag)
         if dress is not None:
             self.DRESS = dress
@@ -223,6 +223,9 @@ class CodeGen(Emitter):
         # 600 KB of SASS, far beyond the instruction caches, and with one warp per scheduler nothing hides the
         # fetch latency; a dozen arithmetic-only functions stay cached (DESIGN.md section 9 NEXT-4).
         self.opcalls = stage and opcalls
+        # every staged value of two or more words starts at an EVEN slot (a skipped slot is kept for a later one-word
+        # value): with the paired fp32 layout of hg_stage.cuh a complex number is then one 8-byte access
+        self.align_pairs = stage and align_pairs
 
     # ------------------------------------------------------------------ value registry / operand access
     def _reg(self, name, ctype, depth, mask=AB, region=None, pol_of=None, hvar=None):
@@ -241,8 +244,15 @@ class CodeGen(Emitter):
         """Slot expression of a staged value (allocated on first use)."""
         if v['slot'] is None:
             r = v['region']
-            v['slot'] = self.n_slots[r]
-            self.n_slots[r] += self._size(v)
+            size = self._size(v)
+            if self.align_pairs and size == 1 and self.holes[r]:
+                v['slot'] = self.holes[r].pop()
+            else:
+                if self.align_pairs and size > 1 and self.n_slots[r] % 2:
+                    self.holes[r].append(self.n_slots[r])
+                    self.n_slots[r] += 1
+                v['slot'] = self.n_slots[r]
+                self.n_slots[r] += size
             self.max_slots[r] = max(self.max_slots[r], self.n_slots[r])
         return str(v['slot']) if v['region'] == 0 else 'L + %d' % v['slot']
 
@@ -292,6 +302,7 @@ class CodeGen(Emitter):
         self.vals = {}
         self.n_slots = [0, 0]
         self.max_slots = [0, 0]
+        self.holes = [[], []]
         self.need_K = set()       # masks whose summed momentum is needed
         self.need_P = set()       # external legs whose momentum is read inside loops (kfromp)
         self.dup_names = set()    # cheap depth-0 values evaluated by both warps of a pair
@@ -327,10 +338,13 @@ class CodeGen(Emitter):
         variants = []
         for vi, (hel, roots) in enumerate(self.variants):
             self.n_slots[1] = 0       # loop-level slots are reused by every static-helicity variant
+            self.holes[1] = []
             variants.append(self._emit_variant(vi, hel, roots, cmat))
         pre = self._preamble()
         out = []
         if self.stage:
+            if self.align_pairs:
+                self.max_slots[0] += self.max_slots[0] % 2
             out.append('  constexpr int L = %d;  // first slot of the loop-level values' % self.max_slots[0])
         out += self._render_shared(pre + self.shared_items, '  ')
         out.append('  T me = T(0);')

@@ -106,6 +106,12 @@ OPCALLS = {9}
 # fp64 5.662 -> 5.539 ms / 1.125 -> 1.100 ms; in fp32 the named barrier is SLOWER (config 5 3.274 -> 3.334 ms,
 # config 4 3.943 -> 4.081 ms), so fp32 keeps __syncthreads (hg_process_impl.cuh me2_event); W + 4 jets: no difference
 NAMED_BARRIER = {4, 5}
+# staged processes whose fp32 staging area keeps the words of an event two by two (csrc/hg_stage.cuh PAIRS), with every
+# value of two or more words at an even slot (gen/emit.py align_pairs): a complex number is one 8-byte shared-memory
+# access.  Not W + 4 jets: its 903 words fill the SM exactly, the padding would cost a team.  bench.py, B200, fp32,
+# dominant kernel per 2^20-event launch: config 5 0.6233 -> 0.6088 ms (LDS + STS 17 % -> 9 % of the instructions of
+# an issue-bound kernel), config 4 0.7000 -> 0.7530 ms (slower: stays with single words)
+STAGE_PAIRS = {5}
 
 
 def build(spec, last=None):
@@ -115,7 +121,8 @@ def build(spec, last=None):
         last = spec.last
     def make(leg):
         cg_ = CodeGen(Diagrams(spec, merge=MERGE).build(leg), stage, spec.pid in KFROMP,
-                      dress=spec.pid not in NO_DRESS, groups=GROUPS.get(spec.pid, 1), opcalls=spec.pid in OPCALLS)
+                      dress=spec.pid not in NO_DRESS, groups=GROUPS.get(spec.pid, 1), opcalls=spec.pid in OPCALLS,
+                      align_pairs=spec.pid in STAGE_PAIRS)
         cg_.count_dg = Diagrams(spec).build(leg)   # Feynman-diagram counts: the unmerged enumeration
         return cg_
 
@@ -232,6 +239,7 @@ struct P%(pid)d {
   static constexpr bool stage_global = %(stage_global)s;  // the staging area is global memory, not shared
   static constexpr int n_split = %(n_split)d;  // warps that share an event of a staged process: pair, or team of four
   static constexpr bool named_barrier = %(named_barrier)s;  // rendezvous per pair / team, not per block (hg_stage.cuh)
+  static constexpr bool stage_pairs = %(stage_pairs)s;  // fp32: staged words two by two, complex numbers in one access
   // hg_integrate_step as phase-space kernel + compaction + |M|^2 kernel per chunk (true) or one fused kernel
   static constexpr bool split_step = %(split_step)s;
   static constexpr double avg_factor = %(avg)s;
@@ -269,6 +277,7 @@ struct P%(pid)d {
            stage_global='true' if spec.pid in STAGE_GLOBAL else 'false',
            n_split=2 * GROUPS.get(spec.pid, 1),
            named_barrier='true' if spec.pid in NAMED_BARRIER else 'false',
+           stage_pairs='true' if spec.pid in STAGE_PAIRS else 'false',
            split_step='true' if (cg.n_stage > 0 or spec.pid in SPLIT_STEP) else 'false', avg=repr(row['avg_factor']),
            me_threads=ME_THREADS.get(spec.pid, 128), n_jets=len(jets), n_leps=len(leps), jets=arr(jets),
            leps=arr(leps), gen_call=gen_call, has_had='true' if had_call else 'false',

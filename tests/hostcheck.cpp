@@ -59,6 +59,8 @@ struct TeamStage {
   Barrier* bar;
   double get(int s) const { return ((volatile double*)b)[s]; }
   void put(int s, double v) const { ((volatile double*)b)[s] = v; }
+  void get2(int s, double& x, double& y) const { x = get(s); y = get(s + 1); }
+  void put2(int s, double x, double y) const { put(s, x); put(s + 1, y); }
   int lo() const { return half; }
   int hi() const { return half + 1; }
   bool own(int h) const { return half + 2 * group == h; }
