@@ -87,3 +87,27 @@ def test_empty_and_limits(api):
     assert abs(got[0] / got[2] - got[1] / got[0]) <= 1e-12 * got[0] / got[2]     # w constant: <w> = <w^2>/<w>
     with pytest.raises(api.HgError):
         api.hg_accumulate_noalloc(api.HG_F64, e, e, None, float('nan'), acc)
+
+
+def test_under_cuda_graph_capture(ctx, api):
+    """What the entry point is for: it can be captured into a CUDA graph (no allocation, no synchronisation, no
+    host-side result) and replayed on new contents of the same buffers."""
+    torch.cuda.set_device(0)
+    precision = api.HG_F64
+    n = 3 * 4096 + 77
+    me, wps, ok = _inputs(ctx, api, precision, 4242, n)
+    acc = torch.zeros((4,), dtype=torch.float64, device='cuda')
+    api.hg_accumulate_noalloc(precision, me, wps, ok, RS, acc)      # set-up (symbol address) outside the capture
+    torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g):
+        api.hg_accumulate_noalloc(precision, me, wps, ok, RS, acc)   # launches go to the capturing stream
+    for first in (4242, 99):
+        me2, wps2, ok2 = _inputs(ctx, api, precision, first, n)
+        me.copy_(me2)
+        wps.copy_(wps2)
+        ok.copy_(ok2)
+        acc.fill_(float('nan'))
+        g.replay()
+        torch.cuda.synchronize()
+        _close(acc.cpu().tolist(), ctx.hg_accumulate(precision, me, wps, ok, RS))
