@@ -25,6 +25,22 @@ HG_HD double habs(double x) { return fabs(x); }
 HG_HD float habs(float x) { return fabsf(x); }
 HG_HD bool hpos(double x) { return x > 0.0; }  // the only comparisons the library makes are "x > 0"
 HG_HD bool hpos(float x) { return x > 0.0f; }
+// x or -x under a run-time flag (the helicity -1 polarisation vector from the staged +1 one): on the device one
+// integer XOR of the sign bit instead of a negation and a select per word (the flag is loop-invariant, the mask too)
+HG_HD double hflip(double x, int flip) {
+#if defined(__CUDA_ARCH__)
+  return __hiloint2double(__double2hiint(x) ^ (flip ? (int)0x80000000 : 0), __double2loint(x));
+#else
+  return flip ? -x : x;
+#endif
+}
+HG_HD float hflip(float x, int flip) {
+#if defined(__CUDA_ARCH__)
+  return __int_as_float(__float_as_int(x) ^ (flip ? (int)0x80000000 : 0));
+#else
+  return flip ? -x : x;
+#endif
+}
 
 template <class T>
 struct cx {

@@ -257,11 +257,9 @@ HG_HD Vc<T> ld_pol(const St& st, int s, int flip) {
   v.c[1] = ld_cx<T>(st, s);
   v.c[2] = ld_cx<T>(st, s + 2);
   v.c[3] = mk<T>(st.get(s + 4), T(0));
-  if (flip) {
-    v.c[1].re = -v.c[1].re;
-    v.c[2].re = -v.c[2].re;
-    v.c[3].re = -v.c[3].re;
-  }
+  v.c[1].re = hflip(v.c[1].re, flip);
+  v.c[2].re = hflip(v.c[2].re, flip);
+  v.c[3].re = hflip(v.c[3].re, flip);
   return v;
 }
 
@@ -271,11 +269,10 @@ template <class T>
 struct Pol;
 template <class T, class St>
 HG_HD Pol<T> ld_pol_lc(const St& st, int s, int flip) {
-  const T sg = flip ? T(-1) : T(1);
   const cx<T> e1 = ld_cx<T>(st, s), e2 = ld_cx<T>(st, s + 2);
-  const T v1r = sg * e1.re, v1i = e1.im, v2r = sg * e2.re, v2i = e2.im;
+  const T v1r = hflip(e1.re, flip), v1i = e1.im, v2r = hflip(e2.re, flip), v2i = e2.im;
   Pol<T> p;
-  p.v3 = sg * st.get(s + 4);
+  p.v3 = hflip(st.get(s + 4), flip);
   p.ur = mk<T>(v1r + v2i, v1i - v2r);
   p.ll = mk<T>(v1r - v2i, v1i + v2r);
   return p;

@@ -29,5 +29,6 @@ inline Cnt hsqrt(Cnt x) { ++Cnt::n(); return Cnt(sqrt(x.v)); }
 inline Cnt hrcp(Cnt x) { ++Cnt::n(); return Cnt(1.0 / x.v); }
 inline Cnt habs(Cnt x) { return Cnt(fabs(x.v)); }
 inline bool hpos(Cnt x) { return x.v > 0.0; }
+inline Cnt hflip(Cnt x, int flip) { return flip ? Cnt(-x.v) : x; }
 
 }  // namespace hg
