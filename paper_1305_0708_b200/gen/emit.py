@@ -529,6 +529,8 @@ class CodeGen(Emitter):
     # shared-memory load (ncu source view: one DADD per flow with the stall samples of a whole LDS latency).
     # Measured for W + 4 jets, 2^18 events: one flow at a time 14.15 ms (fp64) / 5.96 ms (fp32), batches of 4
     # 13.50 / 5.55 ms, batches of 8 13.52 / 5.61 ms.
+    # (The batch as a call of a real function -- offsets at run time, signs as a bit mask -- makes the call sites a
+    # quarter smaller but was measured SLOWER for W + 4 jets: 13.3 -> 15.4 ms in fp64, 5.6 -> 7.5 ms in fp32.)
     ACC_BATCH = 4
     _RE_ACC_SMEM = re.compile(r'^acc_add<T>\(st, A \+ (\d+), T\((-?\d+)\), rb, ib\);$')
 
